@@ -1,0 +1,9 @@
+"""paper_2001_03389_b200 -- B200-native sigma-cut RFI cleaning (librfim) and its Python binding.
+
+The product is the C-ABI library `librfim.so` (include/rfim.h) built from csrc/; `binding` marshals
+arguments to it.  `synth` is the seeded input generator used by tests and bench.  Nothing here
+imports the CPU oracle, and nothing falls back to the CPU.
+"""
+from .binding import (MEAN, MEDIAN, VARIANT_AUTO, VARIANT_GENERIC, VARIANT_STAGED, RfimError, RfimOpts,  # noqa: F401
+                      rfim_freq_sigma_cut, rfim_launch_count, rfim_last_variant, rfim_sigma_cut_host,
+                      rfim_time_sigma_cut, rfim_version)
