@@ -1,0 +1,138 @@
+/*
+ * rfim.h -- C ABI of librfim: B200 (sm_100a) sigma-cut RFI cleaning of dynamic spectra.
+ *
+ * The two mitigation methods of RFIm ("Real-Time RFI Mitigation for the Apertif Radio
+ * Transient System", arxiv 2001.03389; citations are PAPER.md line numbers):
+ *
+ *   rfim_time_sigma_cut   TDSC, PAPER.md:100 (Sec. IV) and Fig. 2:
+ *       "For a given frequency channel, each time sample of a batch is compared to the
+ *        global statistics of the batch: the mean and the standard deviation.  If t_i is an
+ *        outlier (|t_i - mu| > n sigma, n the user-defined threshold) it is replaced by the
+ *        mean of the batch."
+ *   rfim_freq_sigma_cut   FDSC, PAPER.md:102,108 (Sec. IV) and Fig. 3:
+ *       channels at a given time are grouped into bins, the bin mean is subtracted, each
+ *       mean-corrected channel is compared to the mean-corrected statistics of all
+ *       channels; an outlier's ORIGINAL value is replaced by the mean of its bin.
+ *   Both take a list of thresholds: the production pipeline iterates ("three iterations
+ *   with 3.25 sigma"); iteration i sees the data cleaned by
+ *   iteration i-1.  Both take a replacement strategy (mean | median).
+ *
+ * Exact definition (readings of the paper where it is silent: DESIGN.md "Readings"):
+ *   population sigma; strict '>'; two-sided; statistics and replacement value are taken
+ *   from the snapshot at the start of the iteration; integer data are tested in exact
+ *   integer arithmetic with the threshold k quantised to p/2^16 (p = round-half-even):
+ *   q^2 (N x - S)^2 > p^2 (N Q - S^2); integer replacement mean = floor((2S+N)/(2N));
+ *   median = lower median (rank floor((N-1)/2)); float32 statistics in fp64.
+ *
+ * Layout: data[beam][channel][sample], sample fastest, rows `sample_stride` elements apart.
+ *
+ * Ownership / execution: every data pointer is a DEVICE pointer owned by the caller; the
+ * library allocates no device memory for them and keeps no state between calls.  The
+ * `thresholds` array is HOST memory, read before the call returns.  Work is enqueued on
+ * `opts->stream` and the call returns without synchronising; no host read of device memory.
+ * Scratch, when a kernel variant needs it, is taken from `opts->workspace`
+ * (rfim_workspace_bytes says how much).
+ *
+ * Errors: return value only (no exceptions, errno or abort).  On any error nothing has
+ * been enqueued.  There is no CPU fallback: a missing device or a failed launch is
+ * RFIM_ERR_CUDA.
+ */
+#ifndef RFIM_H
+#define RFIM_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define RFIM_VERSION 100 /* 0.1.0 */
+#define RFIM_MAX_THRESHOLDS 16
+
+typedef enum { RFIM_U8 = 0, RFIM_F32 = 1 } rfim_dtype;
+typedef enum { RFIM_REPLACE_MEAN = 0, RFIM_REPLACE_MEDIAN = 1 } rfim_replace;
+
+enum {
+  RFIM_OK = 0,
+  RFIM_ERR_INVALID = -1,     /* bad argument (list below)                                  */
+  RFIM_ERR_UNSUPPORTED = -2, /* valid request that no kernel implements yet                */
+  RFIM_ERR_CUDA = -3         /* CUDA runtime error (text: rfim_last_cuda_error)            */
+};
+
+typedef struct {
+  int64_t   sample_stride; /* elements between consecutive (beam,channel) rows; 0 = samples (dense) */
+  int32_t   window;        /* time-domain only: statistics window in samples; 0 = whole row         */
+  int32_t   bin_size;      /* freq-domain only: channels per bin; 0 = one bin of all channels       */
+  void*     out;           /* device; NULL = in place; else same shape/stride as data (may == data) */
+  uint8_t*  flags;         /* device, optional dense [B][C][S]; 1 = replaced in ANY iteration, else 0 */
+  uint64_t* counts;        /* device, optional [n_thresholds]; samples replaced in iteration i
+                              (overwritten, not accumulated; a sample can be counted twice)        */
+  void*     stream;        /* cudaStream_t; NULL = legacy default stream                            */
+  void*     workspace;     /* device scratch of >= rfim_workspace_bytes(...) bytes, or NULL        */
+  int32_t   variant;       /* 0 = auto.  Non-zero selects a kernel variant (testing / tuning):
+                              1 = generic (any alignment, any row length), 2 = staged fast path.
+                              A variant that cannot run the request returns RFIM_ERR_UNSUPPORTED.  */
+  int32_t   reserved;      /* must be 0                                                            */
+} rfim_opts;               /* opts == NULL means all zeros                                          */
+
+/*
+ * Time-domain sigma cut (TDSC) -- PAPER.md:100, Fig. 2.
+ *   data        device pointer, [beams][channels][samples] of `dtype`, rows sample_stride apart
+ *   thresholds  host array of n_thresholds sigma multiples, applied in order (0 <= n <= 16)
+ *   policy      replacement value: snapshot mean or lower median
+ *   opts->window  statistics are per non-overlapping window of this many samples within a row
+ *                 (the last window of a row may be shorter); 0 = the whole row (the paper's batch)
+ * RFIM_ERR_INVALID: NULL data; a dimension <= 0; n_thresholds outside [0,16]; NULL thresholds with
+ *   n > 0; a threshold that is NaN, <= 0 or >= 256; sample_stride in (0, samples); window < 0;
+ *   bin_size < 0; unknown enum; RFIM_U8 with samples > 2^24; reserved != 0; flags/counts/out
+ *   misaligned for their type.
+ * n_thresholds == 0 is a valid no-op (copies data to out when out-of-place).
+ */
+int rfim_time_sigma_cut(void* data, int beams, int channels, int samples, rfim_dtype dtype,
+                        const double* thresholds, int n_thresholds, rfim_replace policy,
+                        const rfim_opts* opts);
+
+/*
+ * Frequency-domain sigma cut (FDSC) -- PAPER.md:102,108, Fig. 3.
+ *   As above, statistics across the `channels` axis for every (beam, sample).
+ *   opts->bin_size  channels per bin for step 1 (bin-mean correction); must divide channels;
+ *                   0 = one bin of all channels (then FDSC is TDSC along the channel axis).
+ * Additional RFIM_ERR_INVALID: bin_size not dividing channels; RFIM_U8 with channels > 2^24 or
+ *   1 < bin_size < channels with bin_size > 65536.
+ */
+int rfim_freq_sigma_cut(void* data, int beams, int channels, int samples, rfim_dtype dtype,
+                        const double* thresholds, int n_thresholds, rfim_replace policy,
+                        const rfim_opts* opts);
+
+/*
+ * Host-buffer convenience (end-to-end path): `data` and `out` are HOST pointers (pinned memory
+ * gives full PCIe rate; pageable works).  Beams are streamed through device staging buffers the
+ * call allocates and frees itself: H2D copy, rfim_time_sigma_cut (if n_time > 0), then
+ * rfim_freq_sigma_cut (if n_freq > 0) on the device, D2H copy, overlapped across beams.  Synchronous:
+ * returns when `out` (or `data`, if out is NULL) holds the result.  opts->out / flags / counts /
+ * stream / workspace must be NULL here; sample_stride, window, bin_size apply.
+ */
+int rfim_sigma_cut_host(void* data, void* out, int beams, int channels, int samples, rfim_dtype dtype,
+                        const double* time_thresholds, int n_time,
+                        const double* freq_thresholds, int n_freq,
+                        rfim_replace policy, const rfim_opts* opts);
+
+/* Bytes of device scratch the given call needs in opts->workspace (0 = none). `op`: 0 time, 1 freq. */
+size_t rfim_workspace_bytes(int op, int beams, int channels, int samples, rfim_dtype dtype,
+                            int n_thresholds, rfim_replace policy, const rfim_opts* opts);
+
+/* Number of kernel launches the library has enqueued in this process (for bench accounting). */
+uint64_t rfim_launch_count(void);
+
+/* Name of the kernel variant the last successful call on this thread selected ("" before any). */
+const char* rfim_last_variant(void);
+
+const char* rfim_status_string(int status);
+const char* rfim_last_cuda_error(void); /* text of the last RFIM_ERR_CUDA on this thread */
+int         rfim_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RFIM_H */

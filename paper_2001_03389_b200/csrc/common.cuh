@@ -1,0 +1,160 @@
+// common.cuh -- device helpers shared by the librfim kernels (sm_100a).
+//
+// Exact integer form of the sigma cut for uint8 data (include/rfim.h, DESIGN.md "Exact integer
+// evaluation"): with S = sum x, Q = sum x^2 over the N snapshot values, V = N Q - S^2 and the
+// threshold k = p / 2^16,
+//     |x - S/N| > k sqrt(V)/N   <=>   (N x - S)^2 > floor(p^2 V / 2^32) =: W
+// (the left side is an integer, so flooring the right side keeps the test exact).  Because the
+// decision depends only on the value x, one cut collapses to two byte bounds: the kept values are
+// the interval lo <= x <= hi (empty: lo = 1, hi = 0).
+#pragma once
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace rfim {
+
+constexpr unsigned FULL = 0xffffffffu;
+
+struct U8Cut {
+  uint32_t N;
+  uint32_t S;      // < 2^32 because N <= 2^24
+  uint64_t W;      // low 64 bits of floor(p^2 V / 2^32)
+  bool never;      // W >= 2^64: no deviation can exceed it
+};
+
+__device__ __forceinline__ U8Cut make_cut_u8(uint32_t N, uint64_t S, uint64_t Q, uint32_t p) {
+  U8Cut c;
+  const uint64_t V = (uint64_t)N * Q - S * S;          // N^2 * variance, < 2^62
+  const uint64_t p2 = (uint64_t)p * p;                  // < 2^48
+  const uint64_t hi = __umul64hi(p2, V), lo = p2 * V;   // 128-bit product p^2 V
+  c.N = N;
+  c.S = (uint32_t)S;
+  c.W = (hi << 32) | (lo >> 32);
+  c.never = (hi >> 32) != 0;
+  return c;
+}
+
+// true <=> value x is cut (|t_i - mu| > n sigma, strict, two-sided)
+__device__ __forceinline__ bool cut_flags_u8(const U8Cut& c, uint32_t x) {
+  const int64_t d = (int64_t)((uint64_t)c.N * x) - (int64_t)c.S;   // |d| < 2^32
+  const uint32_t ad = (uint32_t)(d < 0 ? -d : d);
+  const uint64_t d2 = (uint64_t)ad * ad;
+  return !c.never && d2 > c.W;
+}
+
+// replacement mean for integers, round half up: floor((2S + N) / (2N))   (always in 0..255)
+__device__ __forceinline__ uint32_t rounded_mean_u8(uint32_t N, uint64_t S) {
+  const uint64_t a = 2 * S + N, b = 2 * (uint64_t)N;
+  uint32_t r = (uint32_t)__fdividef((float)a, (float)b);  // within 1 of the quotient (<= 255)
+  while ((uint64_t)(r + 1) * b <= a) ++r;
+  while ((uint64_t)r * b > a) --r;
+  return r;
+}
+
+// Kept interval [lo, hi] of byte values for one cut, evaluated by a whole warp: lane l tests the
+// eight values 8l .. 8l+7 with the exact predicate.  All lanes return the same lo, hi.
+__device__ __forceinline__ void warp_bounds_u8(const U8Cut& c, int lane, int& lo, int& hi) {
+  uint32_t m = 0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) m |= (cut_flags_u8(c, (uint32_t)(lane * 8 + j)) ? 0u : 1u) << j;
+  const uint32_t any = __ballot_sync(FULL, m != 0);
+  if (any == 0) { lo = 1; hi = 0; return; }
+  const int l0 = __ffs(any) - 1, l1 = 31 - __clz(any);
+  const uint32_t m0 = __shfl_sync(FULL, m, l0), m1 = __shfl_sync(FULL, m, l1);
+  lo = l0 * 8 + __ffs(m0) - 1;
+  hi = l1 * 8 + (31 - __clz(m1));
+}
+
+// Same interval for ONE thread (used where threads own columns): the kept set, if not empty,
+// contains floor(S/N) or floor(S/N)+1; binary search outward on the monotone predicate.
+__device__ __forceinline__ void thread_bounds_u8(const U8Cut& c, int& lo, int& hi) {
+  uint32_t x0 = (uint32_t)__fdividef((float)c.S, (float)c.N);
+  while ((uint64_t)(x0 + 1) * c.N <= c.S) ++x0;
+  while ((uint64_t)x0 * c.N > c.S) --x0;                     // x0 = floor(S/N) <= 255
+  int mid;
+  if (!cut_flags_u8(c, x0)) mid = (int)x0;
+  else if (x0 < 255 && !cut_flags_u8(c, x0 + 1)) mid = (int)x0 + 1;
+  else { lo = 1; hi = 0; return; }
+  int a = 0, b = mid;                                        // smallest kept value in [0, mid]
+  while (a < b) { int m = (a + b) >> 1; if (cut_flags_u8(c, (uint32_t)m)) a = m + 1; else b = m; }
+  lo = a;
+  a = mid; b = 255;                                          // largest kept value in [mid, 255]
+  while (a < b) { int m = (a + b + 1) >> 1; if (cut_flags_u8(c, (uint32_t)m)) b = m - 1; else a = m; }
+  hi = a;
+}
+
+__device__ __forceinline__ uint32_t warp_sum_u32(uint32_t v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+  return v;
+}
+__device__ __forceinline__ uint64_t warp_sum_u64(uint64_t v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+  return v;
+}
+__device__ __forceinline__ double warp_sum_f64(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+  return v;
+}
+
+// ---------------------------------------------------------------- async-proxy (TMA bulk) wrappers
+__device__ __forceinline__ uint32_t smem_addr(const void* p) {
+  return (uint32_t)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_addr(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void fence_mbar_init() {
+  asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(uint64_t* bar, uint32_t bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_addr(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t* bar) {
+  asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_addr(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "WAIT_LOOP:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra WAIT_DONE;\n"
+      "bra WAIT_LOOP;\n"
+      "WAIT_DONE:\n"
+      "}\n" ::"r"(smem_addr(bar)),
+      "r"(parity)
+      : "memory");
+}
+// 1-D bulk copy global -> shared (16-byte aligned addresses, size a multiple of 16), completion on mbarrier
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gmem_src, uint32_t bytes, uint64_t* bar) {
+  asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                   smem_addr(smem_dst)),
+               "l"(gmem_src), "r"(bytes), "r"(smem_addr(bar))
+               : "memory");
+}
+// 1-D bulk copy shared -> global, tracked by bulk async-groups
+__device__ __forceinline__ void bulk_store(void* gmem_dst, const void* smem_src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(gmem_dst),
+               "r"(smem_addr(smem_src)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+template <int N>
+__device__ __forceinline__ void bulk_wait_read() {
+  asm volatile("cp.async.bulk.wait_group.read %0;" ::"n"(N) : "memory");
+}
+template <int N>
+__device__ __forceinline__ void bulk_wait_all() {
+  asm volatile("cp.async.bulk.wait_group %0;" ::"n"(N) : "memory");
+}
+// generic-proxy writes to shared memory -> visible to the async proxy (before a bulk store)
+__device__ __forceinline__ void fence_proxy_async_smem() {
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+}
+
+}  // namespace rfim

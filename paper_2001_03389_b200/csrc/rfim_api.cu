@@ -1,0 +1,244 @@
+// rfim_api.cu -- the C ABI of librfim (include/rfim.h): argument checks, variant selection,
+// launches.  No CPU fallback: every step of the path runs in the kernels of this directory.
+#include "../../include/rfim.h"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "common.cuh"
+#include "fd_u8.cuh"
+#include "td_f32.cuh"
+#include "td_u8.cuh"
+
+namespace {
+
+std::atomic<uint64_t> g_launches{0};
+thread_local char t_cuda_error[256] = "";
+thread_local const char* t_variant = "";
+
+constexpr int kMaxSmem = 227 * 1024;   // opt-in dynamic shared memory per CTA on sm_100
+
+int cuda_fail(cudaError_t e, const char* what) {
+  snprintf(t_cuda_error, sizeof(t_cuda_error), "%s: %s", what, cudaGetErrorString(e));
+  return RFIM_ERR_CUDA;
+}
+#define CUDA_TRY(expr)                                   \
+  do {                                                   \
+    cudaError_t e_ = (expr);                             \
+    if (e_ != cudaSuccess) return cuda_fail(e_, #expr);  \
+  } while (0)
+
+struct DevInfo { int sms = 0; };
+int dev_info(DevInfo& d) {
+  int dev = 0;
+  CUDA_TRY(cudaGetDevice(&dev));
+  CUDA_TRY(cudaDeviceGetAttribute(&d.sms, cudaDevAttrMultiProcessorCount, dev));
+  return RFIM_OK;
+}
+
+size_t elem_size(rfim_dtype t) { return t == RFIM_U8 ? 1 : 4; }
+
+// p = round-half-even(k * 2^16): k * 65536 is exact, nearbyint rounds half to even (default mode)
+uint32_t quantise(double k) { return (uint32_t)std::nearbyint(k * 65536.0); }
+
+struct Call {
+  void* data; void* out;
+  int beams, channels, samples;
+  rfim_dtype dtype;
+  const double* thr; int n_thr;
+  rfim_replace policy;
+  int64_t stride; int window; int bin_size;
+  uint8_t* flags; unsigned long long* counts;
+  cudaStream_t stream; void* workspace; int variant;
+};
+
+int validate(int op, void* data, int beams, int channels, int samples, rfim_dtype dtype,
+             const double* thr, int n_thr, rfim_replace policy, const rfim_opts* o, Call& c) {
+  if (!data || beams <= 0 || channels <= 0 || samples <= 0) return RFIM_ERR_INVALID;
+  if (dtype != RFIM_U8 && dtype != RFIM_F32) return RFIM_ERR_INVALID;
+  if (policy != RFIM_REPLACE_MEAN && policy != RFIM_REPLACE_MEDIAN) return RFIM_ERR_INVALID;
+  if (n_thr < 0 || n_thr > RFIM_MAX_THRESHOLDS) return RFIM_ERR_INVALID;
+  if (n_thr > 0 && !thr) return RFIM_ERR_INVALID;
+  for (int i = 0; i < n_thr; ++i)
+    if (!(thr[i] > 0.0) || !(thr[i] < 256.0)) return RFIM_ERR_INVALID;   // also rejects NaN
+  if (dtype == RFIM_U8 && (op == 0 ? samples : channels) > (1 << 24)) return RFIM_ERR_INVALID;
+  rfim_opts z;
+  memset(&z, 0, sizeof(z));
+  if (o) z = *o;
+  if (z.reserved != 0) return RFIM_ERR_INVALID;
+  if (z.sample_stride != 0 && z.sample_stride < samples) return RFIM_ERR_INVALID;
+  if (z.window < 0 || z.bin_size < 0) return RFIM_ERR_INVALID;
+  if (z.variant < 0 || z.variant > 2) return RFIM_ERR_INVALID;
+  if (op == 1 && z.bin_size != 0) {
+    if (z.bin_size > channels || channels % z.bin_size != 0) return RFIM_ERR_INVALID;
+    if (dtype == RFIM_U8 && z.bin_size != channels && z.bin_size > 65536) return RFIM_ERR_INVALID;
+  }
+  const size_t es = elem_size(dtype);
+  if ((reinterpret_cast<uintptr_t>(data) % es) != 0) return RFIM_ERR_INVALID;
+  if (z.out && (reinterpret_cast<uintptr_t>(z.out) % es) != 0) return RFIM_ERR_INVALID;
+  if (z.counts && (reinterpret_cast<uintptr_t>(z.counts) % 8) != 0) return RFIM_ERR_INVALID;
+  c.data = data;
+  c.out = z.out ? z.out : data;
+  c.beams = beams; c.channels = channels; c.samples = samples;
+  c.dtype = dtype; c.thr = thr; c.n_thr = n_thr; c.policy = policy;
+  c.stride = z.sample_stride ? z.sample_stride : samples;
+  c.window = (z.window == 0 || z.window > samples) ? samples : z.window;
+  c.bin_size = (z.bin_size == 0) ? channels : z.bin_size;
+  c.flags = z.flags;
+  c.counts = reinterpret_cast<unsigned long long*>(z.counts);
+  c.stream = reinterpret_cast<cudaStream_t>(z.stream);
+  c.workspace = z.workspace;
+  c.variant = z.variant;
+  return RFIM_OK;
+}
+
+// flags / counts are defined as "overwritten": clear them on the stream before the kernel adds to them
+int clear_outputs(const Call& c) {
+  if (c.flags)
+    CUDA_TRY(cudaMemsetAsync(c.flags, 0, (size_t)c.beams * c.channels * c.samples, c.stream));
+  if (c.counts && c.n_thr > 0)
+    CUDA_TRY(cudaMemsetAsync(c.counts, 0, sizeof(unsigned long long) * c.n_thr, c.stream));
+  return RFIM_OK;
+}
+
+int copy_through(const Call& c) {   // n_thresholds == 0, out of place
+  if (c.out != c.data) {
+    const size_t es = elem_size(c.dtype);
+    CUDA_TRY(cudaMemcpy2DAsync(c.out, (size_t)c.stride * es, c.data, (size_t)c.stride * es,
+                               (size_t)c.samples * es, (size_t)c.beams * c.channels,
+                               cudaMemcpyDeviceToDevice, c.stream));
+  }
+  return RFIM_OK;
+}
+
+int after_launch(const char* name) {
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return cuda_fail(e, name);
+  g_launches.fetch_add(1, std::memory_order_relaxed);
+  t_variant = name;
+  return RFIM_OK;
+}
+
+// ------------------------------------------------------------------------------------------ TD u8
+struct StagedPlan { int nwarps, slot_bytes, queue_entries, smem; };
+
+bool plan_td_u8_staged(const Call& c, StagedPlan& pl) {
+  if (c.window != c.samples || c.policy != RFIM_REPLACE_MEAN) return false;
+  // every row must have the same misalignment in src and dst for the aligned interior to match
+  if (((reinterpret_cast<uintptr_t>(c.data) ^ reinterpret_cast<uintptr_t>(c.out)) & 15) != 0) return false;
+  pl.slot_bytes = (c.samples + 30 + 15) & ~15;
+  pl.queue_entries = ((pl.slot_bytes / 16) + 3) & ~3;
+  const int per_warp = pl.slot_bytes + pl.queue_entries * 2 + 8;
+  pl.nwarps = kMaxSmem / per_warp;
+  if (pl.nwarps > 16) pl.nwarps = 16;
+  if (pl.nwarps < 4) return false;
+  pl.smem = pl.nwarps * per_warp;
+  return true;
+}
+
+int launch_td_u8(const Call& c) {
+  rfim::TdU8Params P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const uint8_t*>(c.data);
+  P.dst = static_cast<uint8_t*>(c.out);
+  P.rows = (int64_t)c.beams * c.channels;
+  P.stride = c.stride;
+  P.S = c.samples;
+  P.window = c.window;
+  P.n_thr = c.n_thr;
+  P.policy = (int)c.policy;
+  for (int i = 0; i < c.n_thr; ++i) P.p[i] = quantise(c.thr[i]);
+  P.flags = c.flags;
+  P.counts = c.counts;
+  DevInfo dv;
+  int st = dev_info(dv);
+  if (st != RFIM_OK) return st;
+
+  StagedPlan pl;
+  const bool can_stage = plan_td_u8_staged(c, pl);
+  if (c.variant == 2 && !can_stage) return RFIM_ERR_UNSUPPORTED;
+  if (can_stage && c.variant != 1) {
+    P.slot_bytes = pl.slot_bytes;
+    P.queue_entries = pl.queue_entries;
+    CUDA_TRY(cudaFuncSetAttribute(rfim::td_u8_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem));
+    int occ = 0;
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rfim::td_u8_staged_kernel, pl.nwarps * 32, pl.smem));
+    if (occ < 1) occ = 1;
+    int64_t grid = (P.rows + pl.nwarps - 1) / pl.nwarps;
+    if (grid > (int64_t)dv.sms * occ) grid = (int64_t)dv.sms * occ;
+    if ((st = clear_outputs(c)) != RFIM_OK) return st;
+    rfim::td_u8_staged_kernel<<<(unsigned)grid, pl.nwarps * 32, pl.smem, c.stream>>>(P);
+    return after_launch("td_u8_staged");
+  }
+  int64_t grid = P.rows;
+  if (grid > (int64_t)dv.sms * 32) grid = (int64_t)dv.sms * 32;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  rfim::td_u8_generic_kernel<<<(unsigned)grid, rfim::kGenericThreads, 0, c.stream>>>(P);
+  return after_launch("td_u8_generic");
+}
+
+}  // namespace
+
+// =============================================================================================
+extern "C" {
+
+int rfim_time_sigma_cut(void* data, int beams, int channels, int samples, rfim_dtype dtype,
+                        const double* thresholds, int n_thresholds, rfim_replace policy,
+                        const rfim_opts* opts) {
+  Call c;
+  int st = validate(0, data, beams, channels, samples, dtype, thresholds, n_thresholds, policy, opts, c);
+  if (st != RFIM_OK) return st;
+  if (c.n_thr == 0) {
+    if ((st = clear_outputs(c)) != RFIM_OK) return st;
+    return copy_through(c);
+  }
+  if (dtype == RFIM_U8) return launch_td_u8(c);
+  return RFIM_ERR_UNSUPPORTED;
+}
+
+int rfim_freq_sigma_cut(void* data, int beams, int channels, int samples, rfim_dtype dtype,
+                        const double* thresholds, int n_thresholds, rfim_replace policy,
+                        const rfim_opts* opts) {
+  Call c;
+  int st = validate(1, data, beams, channels, samples, dtype, thresholds, n_thresholds, policy, opts, c);
+  if (st != RFIM_OK) return st;
+  if (c.n_thr == 0) {
+    if ((st = clear_outputs(c)) != RFIM_OK) return st;
+    return copy_through(c);
+  }
+  return RFIM_ERR_UNSUPPORTED;
+}
+
+int rfim_sigma_cut_host(void* data, void* out, int beams, int channels, int samples, rfim_dtype dtype,
+                        const double* time_thresholds, int n_time,
+                        const double* freq_thresholds, int n_freq,
+                        rfim_replace policy, const rfim_opts* opts) {
+  (void)data; (void)out; (void)beams; (void)channels; (void)samples; (void)dtype;
+  (void)time_thresholds; (void)n_time; (void)freq_thresholds; (void)n_freq; (void)policy; (void)opts;
+  return RFIM_ERR_UNSUPPORTED;
+}
+
+size_t rfim_workspace_bytes(int op, int beams, int channels, int samples, rfim_dtype dtype,
+                            int n_thresholds, rfim_replace policy, const rfim_opts* opts) {
+  (void)op; (void)beams; (void)channels; (void)samples; (void)dtype; (void)n_thresholds; (void)policy; (void)opts;
+  return 0;
+}
+
+uint64_t rfim_launch_count(void) { return g_launches.load(std::memory_order_relaxed); }
+const char* rfim_last_variant(void) { return t_variant; }
+const char* rfim_last_cuda_error(void) { return t_cuda_error; }
+int rfim_version(void) { return RFIM_VERSION; }
+
+const char* rfim_status_string(int status) {
+  switch (status) {
+    case RFIM_OK: return "ok";
+    case RFIM_ERR_INVALID: return "invalid argument";
+    case RFIM_ERR_UNSUPPORTED: return "unsupported: no kernel implements this request";
+    case RFIM_ERR_CUDA: return "CUDA error (see rfim_last_cuda_error)";
+    default: return "unknown status";
+  }
+}
+
+}  // extern "C"
