@@ -23,9 +23,9 @@ struct U8Cut {
   bool never;      // W >= 2^64: no deviation can exceed it
 };
 
-__device__ __forceinline__ U8Cut make_cut_u8(uint32_t N, uint64_t S, uint64_t Q, uint32_t p) {
+// V = N Q - S^2 = N^2 * variance (< 2^62 for N <= 2^24)
+__device__ __forceinline__ U8Cut make_cut_u8(uint32_t N, uint64_t S, uint64_t V, uint32_t p) {
   U8Cut c;
-  const uint64_t V = (uint64_t)N * Q - S * S;          // N^2 * variance, < 2^62
   const uint64_t p2 = (uint64_t)p * p;                  // < 2^48
   const uint64_t hi = __umul64hi(p2, V), lo = p2 * V;   // 128-bit product p^2 V
   c.N = N;
@@ -45,10 +45,17 @@ __device__ __forceinline__ bool cut_flags_u8(const U8Cut& c, uint32_t x) {
 
 // replacement mean for integers, round half up: floor((2S + N) / (2N))   (always in 0..255)
 __device__ __forceinline__ uint32_t rounded_mean_u8(uint32_t N, uint64_t S) {
-  const uint64_t a = 2 * S + N, b = 2 * (uint64_t)N;
-  uint32_t r = (uint32_t)__fdividef((float)a, (float)b);  // within 1 of the quotient (<= 255)
-  while ((uint64_t)(r + 1) * b <= a) ++r;
+  const uint64_t a = 2 * S + N, b = 2 * (uint64_t)N;      // a < 2^33, b <= 2^25, quotient <= 255
+  uint32_t r = (uint32_t)__fdividef((float)a, (float)b);  // within 1 of the quotient
+  if (r > 255u) r = 255u;
+  if (a < (1ull << 31)) {                                 // 32-bit arithmetic: r b <= a + b < 2^32
+    const uint32_t a32 = (uint32_t)a, b32 = (uint32_t)b;
+    while (r * b32 > a32) --r;
+    while (a32 - r * b32 >= b32) ++r;
+    return r;
+  }
   while ((uint64_t)r * b > a) --r;
+  while (a - (uint64_t)r * b >= b) ++r;
   return r;
 }
 

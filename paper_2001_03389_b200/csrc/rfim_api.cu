@@ -51,7 +51,7 @@ struct Call {
   rfim_replace policy;
   int64_t stride; int window; int bin_size;
   uint8_t* flags; unsigned long long* counts;
-  cudaStream_t stream; void* workspace; int variant;
+  cudaStream_t stream; void* workspace; int variant; int reserved_team;
 };
 
 int validate(int op, void* data, int beams, int channels, int samples, rfim_dtype dtype,
@@ -70,7 +70,7 @@ int validate(int op, void* data, int beams, int channels, int samples, rfim_dtyp
   if (z.reserved != 0) return RFIM_ERR_INVALID;
   if (z.sample_stride != 0 && z.sample_stride < samples) return RFIM_ERR_INVALID;
   if (z.window < 0 || z.bin_size < 0) return RFIM_ERR_INVALID;
-  if (z.variant < 0 || z.variant > 2) return RFIM_ERR_INVALID;
+  if (z.variant < 0 || z.variant > 4) return RFIM_ERR_INVALID;
   if (op == 1 && z.bin_size != 0) {
     if (z.bin_size > channels || channels % z.bin_size != 0) return RFIM_ERR_INVALID;
     if (dtype == RFIM_U8 && z.bin_size != channels && z.bin_size > 65536) return RFIM_ERR_INVALID;
@@ -91,6 +91,8 @@ int validate(int op, void* data, int beams, int channels, int samples, rfim_dtyp
   c.stream = reinterpret_cast<cudaStream_t>(z.stream);
   c.workspace = z.workspace;
   c.variant = z.variant;
+  c.reserved_team = 0;
+  if (z.variant == 3 || z.variant == 4) { c.reserved_team = z.variant - 2; c.variant = 2; }
   return RFIM_OK;
 }
 
@@ -122,19 +124,23 @@ int after_launch(const char* name) {
 }
 
 // ------------------------------------------------------------------------------------------ TD u8
-struct StagedPlan { int nwarps, slot_bytes, queue_entries, smem; };
+struct StagedPlan { int nteams, team, slot_bytes, queue_entries, smem; };
 
 bool plan_td_u8_staged(const Call& c, StagedPlan& pl) {
   if (c.window != c.samples || c.policy != RFIM_REPLACE_MEAN) return false;
   // every row must have the same misalignment in src and dst for the aligned interior to match
   if (((reinterpret_cast<uintptr_t>(c.data) ^ reinterpret_cast<uintptr_t>(c.out)) & 15) != 0) return false;
+  if (c.samples > 65000) return false;                    // 32-bit S, Q totals inside the kernel
   pl.slot_bytes = (c.samples + 30 + 15) & ~15;
   pl.queue_entries = ((pl.slot_bytes / 16) + 3) & ~3;
-  const int per_warp = pl.slot_bytes + pl.queue_entries * 2 + 8;
-  pl.nwarps = kMaxSmem / per_warp;
-  if (pl.nwarps > 16) pl.nwarps = 16;
-  if (pl.nwarps < 4) return false;
-  pl.smem = pl.nwarps * per_warp;
+  // per team: one slot, one hit queue, one control block; sixteen teams keep sixteen rows in flight
+  const int per_team = pl.slot_bytes + pl.queue_entries * 2 + rfim::kCtrlBytes;
+  pl.nteams = kMaxSmem / per_team;
+  if (pl.nteams > 16) pl.nteams = 16;
+  if (pl.nteams < 4) return false;
+  pl.smem = pl.nteams * per_team;
+  pl.team = 1;                                            // warps per row (TD kernel: measured)
+  if (c.variant == 2 && c.reserved_team > 0) pl.team = c.reserved_team;
   return true;
 }
 
@@ -149,7 +155,7 @@ int launch_td_u8(const Call& c) {
   P.window = c.window;
   P.n_thr = c.n_thr;
   P.policy = (int)c.policy;
-  for (int i = 0; i < c.n_thr; ++i) P.p[i] = quantise(c.thr[i]);
+  for (int i = 0; i < c.n_thr; ++i) { P.p[i] = quantise(c.thr[i]); P.pf[i] = (float)P.p[i] * (1.0f / 65536.0f); }
   P.flags = c.flags;
   P.counts = c.counts;
   DevInfo dv;
@@ -162,15 +168,19 @@ int launch_td_u8(const Call& c) {
   if (can_stage && c.variant != 1) {
     P.slot_bytes = pl.slot_bytes;
     P.queue_entries = pl.queue_entries;
-    CUDA_TRY(cudaFuncSetAttribute(rfim::td_u8_staged_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem));
+    void (*kernel)(const rfim::TdU8Params);
+    if (pl.team == 2) kernel = c.flags ? rfim::td_u8_staged_kernel<2, true> : rfim::td_u8_staged_kernel<2, false>;
+    else kernel = c.flags ? rfim::td_u8_staged_kernel<1, true> : rfim::td_u8_staged_kernel<1, false>;
+    const int threads = pl.nteams * pl.team * 32;
+    CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem));
     int occ = 0;
-    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, rfim::td_u8_staged_kernel, pl.nwarps * 32, pl.smem));
+    CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, threads, pl.smem));
     if (occ < 1) occ = 1;
-    int64_t grid = (P.rows + pl.nwarps - 1) / pl.nwarps;
+    int64_t grid = (P.rows + pl.nteams - 1) / pl.nteams;
     if (grid > (int64_t)dv.sms * occ) grid = (int64_t)dv.sms * occ;
     if ((st = clear_outputs(c)) != RFIM_OK) return st;
-    rfim::td_u8_staged_kernel<<<(unsigned)grid, pl.nwarps * 32, pl.smem, c.stream>>>(P);
-    return after_launch("td_u8_staged");
+    kernel<<<(unsigned)grid, threads, pl.smem, c.stream>>>(P);
+    return after_launch(pl.team == 2 ? "td_u8_staged_team2" : "td_u8_staged");
   }
   int64_t grid = P.rows;
   if (grid > (int64_t)dv.sms * 32) grid = (int64_t)dv.sms * 32;

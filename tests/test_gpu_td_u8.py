@@ -61,13 +61,14 @@ def noisy(shape, seed, mu=100, sigma=12):
 
 
 # ----------------------------------------------------------------------------------- configs
-@pytest.mark.parametrize("variant", [rfim.VARIANT_STAGED, rfim.VARIANT_GENERIC])
+@pytest.mark.parametrize("variant", [rfim.VARIANT_STAGED_1W, rfim.VARIANT_STAGED_2W, rfim.VARIANT_GENERIC])
 def test_config1_tiny(variant):
     """BASELINE.json configs[0]: 1 x 64 x 1024, k = 3, mean."""
     cfg = synth.config(1)
     x = synth.fill_host(cfg)
     name, counts = check(x, cfg["thresholds"], variant=variant)
-    assert name == ("td_u8_staged" if variant == rfim.VARIANT_STAGED else "td_u8_generic")
+    assert name == {rfim.VARIANT_STAGED_1W: "td_u8_staged", rfim.VARIANT_STAGED_2W: "td_u8_staged_team2",
+                    rfim.VARIANT_GENERIC: "td_u8_generic"}[variant]
     # P13: the 3 broadband spikes (+80 = 8 sigma) on all 64 channels are cut ...
     d = synth.Descriptor(cfg)
     spikes = np.nonzero(d.imp_amp[0])[0]
@@ -87,6 +88,7 @@ def test_config2_arts_like_all_beams():
     x_np = x.cpu().numpy()
     name, counts = check(x_np, cfg["thresholds"], inplace=True)
     assert name == "td_u8_staged"
+    check(x_np[:2], cfg["thresholds"], variant=rfim.VARIANT_STAGED_2W)
     assert all(int(c) > 0 for c in counts)
 
 
@@ -99,7 +101,7 @@ def test_device_generator_matches_host_twin():
 
 # --------------------------------------------------------------------- shapes, tails, alignment
 @pytest.mark.parametrize("S", [1, 2, 15, 16, 17, 31, 33, 100, 255, 1000, 4099, 12500])
-@pytest.mark.parametrize("variant", [rfim.VARIANT_STAGED, rfim.VARIANT_GENERIC])
+@pytest.mark.parametrize("variant", [rfim.VARIANT_STAGED_1W, rfim.VARIANT_STAGED_2W, rfim.VARIANT_GENERIC])
 def test_row_lengths_and_misalignment(S, variant):
     """Odd S makes consecutive rows start at every 16-byte phase; several 16-byte groups and a ragged tail."""
     x = noisy((2, 19, S), seed=S)
@@ -113,7 +115,7 @@ def test_row_lengths_and_misalignment(S, variant):
     check(x, [3.25, 3.25, 3.25], variant=variant, inplace=True)
 
 
-@pytest.mark.parametrize("variant", [rfim.VARIANT_STAGED, rfim.VARIANT_GENERIC])
+@pytest.mark.parametrize("variant", [rfim.VARIANT_STAGED_1W, rfim.VARIANT_STAGED_2W, rfim.VARIANT_GENERIC])
 @pytest.mark.parametrize("pitch", [1040, 1027])
 def test_padded_pitch(variant, pitch):
     x = noisy((3, 8, 1000), seed=11)
@@ -140,7 +142,7 @@ def test_misaligned_out_falls_back_to_generic():
 
 
 # ----------------------------------------------------------------------------- degenerate data
-@pytest.mark.parametrize("variant", [rfim.VARIANT_STAGED, rfim.VARIANT_GENERIC])
+@pytest.mark.parametrize("variant", [rfim.VARIANT_STAGED_1W, rfim.VARIANT_STAGED_2W, rfim.VARIANT_GENERIC])
 def test_degenerate_rows(variant):
     S = 777
     x = np.zeros((1, 10, S), dtype=np.uint8)
@@ -162,7 +164,7 @@ def test_worked_example_p3_on_gpu():
     """15 x 100 and one 160, k = {3,3,3} -> 104 -> 100 (hand-computed in tests/test_oracle_pins.py)."""
     x = np.full((1, 1, 16), 100, dtype=np.uint8)
     x[0, 0, 5] = 160
-    for variant in (rfim.VARIANT_STAGED, rfim.VARIANT_GENERIC):
+    for variant in (rfim.VARIANT_STAGED_1W, rfim.VARIANT_STAGED_2W, rfim.VARIANT_GENERIC):
         got, flags, counts, _ = run_gpu(x, [3.0, 3.0, 3.0], variant=variant)
         assert got[0, 0].tolist() == [100] * 16 and counts.tolist() == [1, 1, 0]
         got, _, counts, _ = run_gpu(x, [3.0], variant=variant)
@@ -180,7 +182,7 @@ def test_heavy_rfi_rows(ks):
     x[0, 3, : S // 3] = 0
     x[0, 4, 100:4900] = 200
     x[0, 5, :] = np.where(np.arange(S) % 50 < 3, 250, x[0, 5, :])
-    for variant in (rfim.VARIANT_STAGED, rfim.VARIANT_GENERIC):
+    for variant in (rfim.VARIANT_STAGED_1W, rfim.VARIANT_STAGED_2W, rfim.VARIANT_GENERIC):
         check(x, ks, variant=variant)
 
 
@@ -224,7 +226,8 @@ def test_many_rows_grid_wraps():
     """More rows than resident warps: the persistent loop and slot reuse (mbarrier phase, bulk groups)."""
     x = noisy((4, 3000, 257), seed=71)
     x[:, ::5, 100] = 255
-    check(x, [4.0, 3.0], variant=rfim.VARIANT_STAGED)
+    check(x, [4.0, 3.0], variant=rfim.VARIANT_STAGED_1W)
+    check(x, [4.0, 3.0], variant=rfim.VARIANT_STAGED_2W)
 
 
 def test_other_stream():
