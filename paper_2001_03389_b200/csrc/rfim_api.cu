@@ -189,6 +189,161 @@ int launch_td_u8(const Call& c) {
   return after_launch("td_u8_generic");
 }
 
+// ------------------------------------------------------------------------------------------ FD u8
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+struct FdPlan { int ts, m, rows_per_class, box_rows, smem; bool exact; };
+
+template <int Ts, bool kExact>
+size_t fd_smem_bytes(int C) {
+  const size_t row_bytes = kExact ? Ts : Ts + 16;
+  return (((size_t)C * row_bytes + 127) & ~(size_t)127) + sizeof(rfim::FdSmem<Ts>);
+}
+size_t fd_smem_for(int ts, int C) {
+  switch (ts) {
+    case 128: return fd_smem_bytes<128, true>(C);
+    case 64: return fd_smem_bytes<64, true>(C);
+    case 32: return fd_smem_bytes<32, true>(C);
+    case 112: return fd_smem_bytes<112, false>(C);
+    default: return fd_smem_bytes<48, false>(C);
+  }
+}
+
+// Tile geometry for the request, or false when only the generic kernel can run it.  `big` prefers the
+// widest tile that fits one CTA per SM over a narrower one with two CTAs per SM (variant 3).
+bool plan_fd_u8_tile(const Call& c, bool big, FdPlan& pl) {
+  if (c.policy != RFIM_REPLACE_MEAN || c.bin_size != c.channels) return false;
+  int m = 1;
+  while ((((int64_t)m * c.stride) & 15) != 0) m <<= 1;       // rows per 16-byte alignment period
+  if (m > rfim::kFdMaxClasses || c.channels % m != 0) return false;
+  if (c.channels > 60000) return false;                      // 32-bit column totals inside the kernel
+  const uintptr_t src = reinterpret_cast<uintptr_t>(c.data), dst = reinterpret_cast<uintptr_t>(c.out);
+  pl.exact = (m == 1) && ((src | dst) & 15) == 0;
+  if (!pl.exact && ((src | dst) & 3) != 0) return false;     // 32-bit stores of the tile
+  pl.m = m;
+  pl.rows_per_class = c.channels / m;
+  static const int exact_ts[3] = {128, 64, 32}, over_ts[2] = {112, 48};
+  const int* cand = pl.exact ? exact_ts : over_ts;
+  const int ncand = pl.exact ? 3 : 2;
+  const size_t half = (size_t)(kMaxSmem + 1024) / 2 - 1024;  // two CTAs per SM (1 KB reserved per CTA)
+  // TMA boxes: rows per box divides the class, <= 256, and every box lands 128-byte aligned in shared memory
+  auto boxes_for = [&](int ts) {
+    const int row_bytes = pl.exact ? ts : ts + 16;
+    if (m > 1 && ((int64_t)pl.rows_per_class * row_bytes) % 128 != 0) return 0;
+    int best = 0;
+    for (int d = 1; d <= 256 && d <= pl.rows_per_class; ++d)
+      if (pl.rows_per_class % d == 0 && (d * row_bytes) % 128 == 0) best = d;
+    if (pl.rows_per_class == best) return best;                // a single box needs no alignment of its size
+    if (best == 0 && pl.rows_per_class <= 256) return pl.rows_per_class;
+    return (best && pl.rows_per_class / best <= 64) ? best : 0;
+  };
+  pl.ts = 0;
+  for (int pass = big ? 1 : 0; pass < 2 && !pl.ts; ++pass)
+    for (int i = 0; i < ncand && !pl.ts; ++i)
+      if (fd_smem_for(cand[i], c.channels) <= (pass == 0 ? half : (size_t)kMaxSmem) && boxes_for(cand[i]) > 0)
+        pl.ts = cand[i];
+  if (!pl.ts) return false;
+  pl.box_rows = boxes_for(pl.ts);
+  pl.smem = (int)fd_smem_for(pl.ts, c.channels);
+  return true;
+}
+
+// one 2-D tensor per alignment class r: rows r, r+m, r+2m, ... of the [beams*channels][pitch] matrix,
+// origin rounded down to 16 bytes (off[r] bytes before the row start)
+bool encode_fd_maps(const Call& c, const FdPlan& pl, uint8_t* base, CUtensorMap* maps, int* off) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  for (int r = 0; r < pl.m; ++r) {
+    const uintptr_t addr = reinterpret_cast<uintptr_t>(base) + (uintptr_t)r * (uintptr_t)c.stride;
+    off[r] = (int)(addr & 15);
+    cuuint64_t dims[2] = {(cuuint64_t)c.samples + (cuuint64_t)off[r],
+                          (cuuint64_t)c.beams * (cuuint64_t)pl.rows_per_class};
+    cuuint64_t strides[1] = {(cuuint64_t)pl.m * (cuuint64_t)c.stride};
+    cuuint32_t box[2] = {(cuuint32_t)(pl.exact ? pl.ts : pl.ts + 16), (cuuint32_t)pl.box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    if (enc(&maps[r], CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, reinterpret_cast<void*>(addr - off[r]), dims, strides, box,
+            estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+  }
+  return true;
+}
+
+template <int Ts, bool kExact>
+int launch_fd_tile(const Call& c, const FdPlan& pl, const rfim::FdMaps& maps, rfim::FdU8Params& P, int sms,
+                   const char* name) {
+  auto kernel = rfim::fd_u8_tile_kernel<Ts, kExact>;
+  CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem));
+  int occ = 0;
+  CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, 4 * Ts, pl.smem));
+  if (occ < 1) occ = 1;
+  int64_t grid = P.total_tiles;
+  if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
+  int st = clear_outputs(c);
+  if (st != RFIM_OK) return st;
+  kernel<<<(unsigned)grid, 4 * Ts, pl.smem, c.stream>>>(maps, P);
+  return after_launch(name);
+}
+
+int launch_fd_u8(const Call& c) {
+  rfim::FdU8Params P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const uint8_t*>(c.data);
+  P.dst = static_cast<uint8_t*>(c.out);
+  P.stride = c.stride;
+  P.beams = c.beams; P.C = c.channels; P.S = c.samples;
+  P.n_thr = c.n_thr;
+  for (int i = 0; i < c.n_thr; ++i) { P.p[i] = quantise(c.thr[i]); P.pf[i] = (float)P.p[i] * (1.0f / 65536.0f); }
+  P.flags = c.flags;
+  P.counts = c.counts;
+  DevInfo dv;
+  int st = dev_info(dv);
+  if (st != RFIM_OK) return st;
+
+  FdPlan pl;
+  bool can_tile = c.variant != 1 && plan_fd_u8_tile(c, c.reserved_team == 1, pl);
+  rfim::FdMaps maps;
+  if (can_tile) {
+    int off_dst[rfim::kFdMaxClasses] = {0, 0, 0, 0};
+    can_tile = encode_fd_maps(c, pl, static_cast<uint8_t*>(c.data), maps.src, P.off) &&
+               (!pl.exact || encode_fd_maps(c, pl, static_cast<uint8_t*>(c.out), maps.dst, off_dst));
+  }
+  if (c.variant == 2 && !can_tile) return RFIM_ERR_UNSUPPORTED;
+  if (can_tile) {
+    P.m = pl.m; P.rows_per_class = pl.rows_per_class; P.box_rows = pl.box_rows;
+    P.tiles_per_beam = (c.samples + pl.ts - 1) / pl.ts;
+    P.total_tiles = (int64_t)P.tiles_per_beam * c.beams;
+    switch (pl.ts) {
+      case 128: return launch_fd_tile<128, true>(c, pl, maps, P, dv.sms, "fd_u8_tile128");
+      case 64: return launch_fd_tile<64, true>(c, pl, maps, P, dv.sms, "fd_u8_tile64");
+      case 32: return launch_fd_tile<32, true>(c, pl, maps, P, dv.sms, "fd_u8_tile32");
+      case 112: return launch_fd_tile<112, false>(c, pl, maps, P, dv.sms, "fd_u8_tile112x");
+      default: return launch_fd_tile<48, false>(c, pl, maps, P, dv.sms, "fd_u8_tile48x");
+    }
+  }
+  if (c.policy != RFIM_REPLACE_MEAN || c.bin_size != c.channels) return RFIM_ERR_UNSUPPORTED;
+  const int64_t ncol = (int64_t)c.beams * c.samples;
+  int64_t grid = (ncol + rfim::kFdGenericThreads - 1) / rfim::kFdGenericThreads;
+  if (grid > (int64_t)dv.sms * 16) grid = (int64_t)dv.sms * 16;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  rfim::fd_u8_generic_kernel<<<(unsigned)grid, rfim::kFdGenericThreads, 0, c.stream>>>(P);
+  return after_launch("fd_u8_generic");
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -218,6 +373,7 @@ int rfim_freq_sigma_cut(void* data, int beams, int channels, int samples, rfim_d
     if ((st = clear_outputs(c)) != RFIM_OK) return st;
     return copy_through(c);
   }
+  if (dtype == RFIM_U8) return launch_fd_u8(c);
   return RFIM_ERR_UNSUPPORTED;
 }
 
