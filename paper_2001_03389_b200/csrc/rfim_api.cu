@@ -381,9 +381,69 @@ int rfim_sigma_cut_host(void* data, void* out, int beams, int channels, int samp
                         const double* time_thresholds, int n_time,
                         const double* freq_thresholds, int n_freq,
                         rfim_replace policy, const rfim_opts* opts) {
-  (void)data; (void)out; (void)beams; (void)channels; (void)samples; (void)dtype;
-  (void)time_thresholds; (void)n_time; (void)freq_thresholds; (void)n_freq; (void)policy; (void)opts;
-  return RFIM_ERR_UNSUPPORTED;
+  // validate exactly as the device entry points do (the host pointers are never dereferenced here)
+  Call ct, cf;
+  int st = validate(0, data, beams, channels, samples, dtype, time_thresholds, n_time, policy, opts, ct);
+  if (st != RFIM_OK) return st;
+  st = validate(1, data, beams, channels, samples, dtype, freq_thresholds, n_freq, policy, opts, cf);
+  if (st != RFIM_OK) return st;
+  if (opts && (opts->out || opts->flags || opts->counts || opts->stream || opts->workspace)) return RFIM_ERR_INVALID;
+  if (!out) out = data;
+  const size_t es = elem_size(dtype);
+  const int64_t stride = ct.stride;
+  const size_t beam_elems = (size_t)channels * (size_t)stride;
+  // chunk of whole beams, about 128 MiB: long enough copies for full PCIe rate, short enough to overlap
+  int per_chunk = (int)((size_t)(128u << 20) / (beam_elems * es));
+  if (per_chunk < 1) per_chunk = 1;
+  if (per_chunk > beams) per_chunk = beams;
+  const int nchunks = (beams + per_chunk - 1) / per_chunk;
+  constexpr int kSlots = 3;
+  const int nslots = nchunks < kSlots ? nchunks : kSlots;
+  void* dev[kSlots] = {nullptr, nullptr, nullptr};
+  cudaStream_t streams[kSlots] = {nullptr, nullptr, nullptr};
+  int rc = RFIM_OK;
+  auto fail = [&](cudaError_t e, const char* what) { if (rc == RFIM_OK) rc = cuda_fail(e, what); };
+  for (int i = 0; i < nslots && rc == RFIM_OK; ++i) {
+    cudaError_t e = cudaMalloc(&dev[i], (size_t)per_chunk * beam_elems * es);
+    if (e != cudaSuccess) { fail(e, "cudaMalloc(staging)"); break; }
+    e = cudaStreamCreateWithFlags(&streams[i], cudaStreamNonBlocking);
+    if (e != cudaSuccess) fail(e, "cudaStreamCreate");
+  }
+  rfim_opts o;
+  memset(&o, 0, sizeof(o));
+  if (opts) { o.sample_stride = opts->sample_stride; o.window = opts->window; o.bin_size = opts->bin_size; }
+  for (int ch = 0; ch < nchunks && rc == RFIM_OK; ++ch) {
+    const int slot = ch % nslots;
+    const int b0 = ch * per_chunk;
+    const int nb = (beams - b0 < per_chunk) ? beams - b0 : per_chunk;
+    const size_t rows = (size_t)nb * channels;
+    const char* h_in = static_cast<const char*>(data) + (size_t)b0 * beam_elems * es;
+    char* h_out = static_cast<char*>(out) + (size_t)b0 * beam_elems * es;
+    cudaError_t e = cudaMemcpy2DAsync(dev[slot], (size_t)stride * es, h_in, (size_t)stride * es, (size_t)samples * es,
+                                      rows, cudaMemcpyHostToDevice, streams[slot]);
+    if (e != cudaSuccess) { fail(e, "cudaMemcpy2DAsync(H2D)"); break; }
+    o.stream = streams[slot];
+    if (n_time > 0) {
+      st = rfim_time_sigma_cut(dev[slot], nb, channels, samples, dtype, time_thresholds, n_time, policy, &o);
+      if (st != RFIM_OK) { rc = st; break; }
+    }
+    if (n_freq > 0) {
+      st = rfim_freq_sigma_cut(dev[slot], nb, channels, samples, dtype, freq_thresholds, n_freq, policy, &o);
+      if (st != RFIM_OK) { rc = st; break; }
+    }
+    e = cudaMemcpy2DAsync(h_out, (size_t)stride * es, dev[slot], (size_t)stride * es, (size_t)samples * es, rows,
+                          cudaMemcpyDeviceToHost, streams[slot]);
+    if (e != cudaSuccess) { fail(e, "cudaMemcpy2DAsync(D2H)"); break; }
+  }
+  for (int i = 0; i < nslots; ++i) {
+    if (streams[i]) {
+      cudaError_t e = cudaStreamSynchronize(streams[i]);
+      if (e != cudaSuccess) fail(e, "cudaStreamSynchronize");
+      cudaStreamDestroy(streams[i]);
+    }
+    if (dev[i]) cudaFree(dev[i]);
+  }
+  return rc;
 }
 
 size_t rfim_workspace_bytes(int op, int beams, int channels, int samples, rfim_dtype dtype,
