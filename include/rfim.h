@@ -71,8 +71,9 @@ typedef struct {
   void*     stream;        /* cudaStream_t; NULL = legacy default stream                            */
   void*     workspace;     /* device scratch of >= rfim_workspace_bytes(...) bytes, or NULL        */
   int32_t   variant;       /* 0 = auto.  Non-zero selects a kernel variant (testing / tuning):
-                              1 = generic (any alignment, any row length), 2 = staged fast path,
-                              3 / 4 = staged with one / two warps per row (time-domain uint8).
+                              1 = generic (any alignment, any row length), 2 = fast path (staged TDSC /
+                              cluster FDSC), 3 / 4 = staged TDSC with one / two warps per row,
+                              5 / 6 / 7 / 8 = cluster FDSC with 1 / 2 / 4 / 8 CTAs per tile.
                               A variant that cannot run the request returns RFIM_ERR_UNSUPPORTED.  */
   int32_t   reserved;      /* must be 0                                                            */
 } rfim_opts;               /* opts == NULL means all zeros                                          */

@@ -18,6 +18,7 @@ MEAN, MEDIAN = 0, 1
 OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_CUDA = 0, -1, -2, -3
 VARIANT_AUTO, VARIANT_GENERIC, VARIANT_STAGED = 0, 1, 2
 VARIANT_STAGED_1W, VARIANT_STAGED_2W = 3, 4
+VARIANT_FD_CL1, VARIANT_FD_CL2, VARIANT_FD_CL4, VARIANT_FD_CL8 = 5, 6, 7, 8
 
 EXPORTS = ("rfim_time_sigma_cut", "rfim_freq_sigma_cut", "rfim_sigma_cut_host", "rfim_workspace_bytes",
            "rfim_launch_count", "rfim_last_variant", "rfim_status_string", "rfim_last_cuda_error",

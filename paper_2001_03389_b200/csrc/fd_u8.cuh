@@ -2,39 +2,36 @@
 // one bin of all channels (BASELINE.json configs[2]).
 //
 // Two kernels:
-//   fd_u8_tile_kernel   the hot path.  A CTA owns a tile of all C channels x Ts consecutive samples of
-//       one beam.  F1: the tile is brought into shared memory by TMA tensor copies issued by one thread.
-//       Rows of a dense [C][S] beam are only 4-byte aligned (12500 mod 16 = 4) while a tensor map needs
-//       16-byte strides AND 16-byte aligned box starts (measured: a box whose inner coordinate is not a
-//       multiple of 16 bytes faults).  So the rows are split into m = 16/gcd(pitch,16) alignment classes
-//       (row mod m): class r is a 2-D tensor with row stride m*pitch whose base is rounded DOWN to 16
-//       bytes (by off_r bytes), and every box is 16 bytes wider than the tile (kExact = false): the
-//       wanted samples sit off_r bytes into each shared-memory row.  When every row is 16-byte aligned
-//       (padded pitch; kExact = true) the boxes are exact and the tile is also stored by TMA.
-//       F2: a thread owns one 32-bit word column (4 samples) and every 16th row; 4x4 byte transposes
-//       (PRMT) turn four rows into four words that each hold ONE column, so that IDP.4A gives the exact
-//       column sums and sums of squares.  F3: one thread per column evaluates the exact integer
-//       predicate around a float estimate -> [lo, hi], r.  F4: packed range check with per-column bounds
-//       (VIADDMNMX.U16x2, 3 instructions per word, eight rows per test); only groups with a hit are
-//       revisited byte by byte (replace in shared memory, update the column's S, Q, count with
-//       shared-memory atomics).  F5: next threshold, on chip.  F6: TMA tensor stores (kExact) or
-//       coalesced 32-bit stores of exactly the tile's bytes.  HBM sees one read and one write per sample.
+//   fd_u8_cluster_kernel   the hot path.  A thread-block CLUSTER of CL CTAs owns a tile of all C
+//       channels x Ts consecutive samples of one beam; CTA q of the cluster holds channels
+//       [q*Rq, (q+1)*Rq) of the tile in its shared memory.  Splitting the channels over a cluster is
+//       what lets the row segments be long (Ts ~ 500 bytes for C = 1536, CL = 8): FDSC wants whole
+//       columns on chip while HBM wants long contiguous rows.
+//       F1: every row segment is one 1-D TMA bulk copy (cp.async.bulk) of the 16-byte aligned
+//       superset of its bytes, issued by one thread per row, all completing on one mbarrier.  Rows of
+//       a dense [C][S] beam are only 4-byte aligned (12500 mod 16 = 4), so row r lands off_r =
+//       (address mod 16) bytes into its shared-memory row; off_r is constant for the rows one thread
+//       owns (they are 4 apart and 4 * pitch is a multiple of 16).
+//       F2: a thread owns one 32-bit word column (4 samples) and every 4th row of the CTA; 4x4 byte
+//       transposes (PRMT) turn four rows into four words that each hold ONE column, so IDP.4A gives
+//       exact column sums and sums of squares.  Partial sums are reduced over the four row groups by
+//       shuffles and over the cluster through distributed shared memory (DSMEM).
+//       F3: column c is owned by one thread of one CTA of the cluster, which keeps (S, Q) in
+//       registers over the iterations, evaluates the exact integer predicate around a float estimate
+//       -> [lo, hi], r, and publishes them (with packed range-check constants); the other CTAs pull
+//       them through DSMEM.
+//       F4: packed range check with per-column bounds (VIADDMNMX.U16x2, 3 instructions per word);
+//       only words with a hit are revisited with exact byte masks (replace in shared memory,
+//       accumulate the column deltas in packed registers).  F5: next threshold, on chip.
+//       F6: every row segment is stored by one bulk copy of its 16-byte aligned interior plus a few
+//       32-bit / byte stores for the ragged ends.  HBM sees one read and one write per sample.
 //   fd_u8_generic_kernel  any pitch / alignment / channel count: one thread per (beam, sample) column,
 //       iterations through global memory (L2).  Correctness path, not tuned.
 #pragma once
 
-#include <cuda.h>   // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
-
 #include "common.cuh"
 
 namespace rfim {
-
-constexpr int kFdMaxClasses = 4;
-
-struct FdMaps {
-  CUtensorMap src[kFdMaxClasses];
-  CUtensorMap dst[kFdMaxClasses];
-};
 
 struct FdU8Params {
   const uint8_t* src;
@@ -46,36 +43,63 @@ struct FdU8Params {
   float pf[16];
   uint8_t* flags;               // optional [beams][C][S]
   unsigned long long* counts;   // optional [n_thr]
-  // tile kernel
-  int m;                        // alignment classes
-  int rows_per_class;           // C / m
-  int box_rows;                 // rows per TMA box (divides rows_per_class, <= 256)
-  int off[kFdMaxClasses];       // x offset (bytes) of class r inside its 16-byte aligned tensor
+  // cluster kernel
+  int Ts;                       // tile width in samples (multiple of 4, <= 4*PW - 16)
+  int WC;                       // word columns per tile, rounded up to a multiple of 8; blockDim = 4*WC
+  int Rq;                       // channels per CTA = ceil(C / cluster size)
   int tiles_per_beam;
   int64_t total_tiles;
 };
-
-// ---------------------------------------------------------------- TMA tensor copies (2-D, tiled)
-__device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
-  asm volatile(
-      "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
-      ::"r"(smem_addr(smem_dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(x), "r"(y), "r"(smem_addr(bar))
-      : "memory");
-}
-__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int x, int y, const void* smem_src) {
-  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];" ::"l"(
-                   reinterpret_cast<uint64_t>(map)),
-               "r"(x), "r"(y), "r"(smem_addr(smem_src))
-               : "memory");
-}
-__device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap* map) {
-  asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(map)) : "memory");
-}
 
 __device__ __forceinline__ uint32_t prmt_b32(uint32_t a, uint32_t b, uint32_t sel) {
   uint32_t d;
   asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
   return d;
+}
+
+// ---------------------------------------------------------------- cluster helpers
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t cluster_nctarank() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t cluster_id_x() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r));
+  return r;
+}
+__device__ __forceinline__ uint32_t cluster_nid_x() {
+  uint32_t r;
+  asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(r));
+  return r;
+}
+// barrier over all threads of all CTAs of the cluster; orders shared-memory accesses cluster-wide
+__device__ __forceinline__ void cluster_sync_all() {
+  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+// address of the same shared-memory location in CTA `rank` of the cluster
+__device__ __forceinline__ uint32_t dsmem_addr(const void* local, uint32_t rank) {
+  uint32_t ra;
+  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(smem_addr(local)), "r"(rank));
+  return ra;
+}
+__device__ __forceinline__ uint32_t dsmem_ld_u32(uint32_t addr) {
+  uint32_t v;
+  asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  return v;
+}
+__device__ __forceinline__ uint4 dsmem_ld_u128(uint32_t addr) {
+  uint4 v;
+  asm volatile("ld.shared::cluster.v4.u32 {%0, %1, %2, %3}, [%4];"
+               : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w)
+               : "r"(addr)
+               : "memory");
+  return v;
 }
 
 // Kept interval for one cut, ONE thread: float estimate of mu -/+ k sigma, then a short walk on the
@@ -112,71 +136,93 @@ __device__ __forceinline__ uint32_t bytes_outside_cols(uint32_t w, uint32_t chiE
   return prmt_b32(fe, fo, 0xFBD9u);
 }
 
-// shared-memory control block behind the tile
-constexpr int kFdRG = 16;                    // row groups: a thread owns every 16th row of each class
-template <int Ts>
-struct FdSmem {
-  static constexpr int WC = Ts / 4;          // word columns
-  uint64_t bar;
-  uint32_t red[kFdRG * WC * 8];              // per row group, per word column: S[4], Q[4]
-  uint32_t dS[Ts], dQ[Ts], dcnt[Ts];         // per column updates of one iteration (atomics)
-  uint32_t lo4[WC], hi4[WC], r4[WC];         // per word column: packed bounds and replacement values
-  uint32_t any_cut;                          // some column of the tile has bounds inside 0..255
-};
+// ---------------------------------------------------------------- cluster kernel
+// Shared memory of one CTA (PW = row pitch in 32-bit words, PW mod 32 in {8, 24} so that the four row
+// groups of a warp fall into disjoint banks; TsP = 4 * WC padded columns):
+//   tile  [Rq][PW] words      the CTA's channels of the tile
+//   xS, xQ [TsP] u32          exchange: this CTA's partial column sums, later its column deltas
+//   chk   [WC] uint4          per word column {negE, negO, thrE, thrO}: packed range-check constants
+//   lo, hi, rr [TsP] bytes    per column kept interval and replacement (exact fix path)
+//   bar, misc
+constexpr int kFdRG = 4;   // row groups: a thread owns rows rg, rg + 4, ... of its CTA
 
-// Ts samples per tile; 4*Ts threads (Ts/4 word columns x 16 row groups).  kExact: rows are 16-byte
-// aligned, boxes are exactly Ts wide and the tile is stored by TMA; else boxes are Ts+16 wide.
-template <int Ts, bool kExact>
-__global__ void __launch_bounds__(4 * Ts) fd_u8_tile_kernel(const __grid_constant__ FdMaps maps, const FdU8Params P) {
-  using Sm = FdSmem<Ts>;
-  constexpr int WC = Sm::WC, RG = kFdRG, NT = 4 * Ts;
-  constexpr int PW = kExact ? WC : WC + 4;                                // shared-memory row pitch in words
+__host__ __device__ inline size_t fd_cluster_ctrl_bytes(int WC) { return (size_t)WC * 4 * 15 + 64; }
+__host__ __device__ inline size_t fd_cluster_smem_bytes(int PW, int Rq, int WC) {
+  return (size_t)Rq * PW * 4 + fd_cluster_ctrl_bytes(WC);
+}
+
+template <int PW>
+__global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params P) {
   extern __shared__ __align__(128) uint8_t smem[];
-  const int C = P.C, Rc = P.rows_per_class;
-  uint32_t* tile = reinterpret_cast<uint32_t*>(smem);                     // [C][PW] words, class-major rows
-  Sm& sm = *reinterpret_cast<Sm*>(smem + (((size_t)C * PW * 4 + 127) & ~(size_t)127));
-  const int tid = threadIdx.x;
-  const int wc = tid % WC, rg = tid / WC;
-  const int nk = (Rc - rg + RG - 1) / RG;             // rows rg, rg+RG, ... of this thread inside EACH class
-  // word offset of the tile's first sample inside a shared-memory row of class r
-  auto wofs = [&](int r) { return kExact ? 0 : (P.off[r] >> 2); };
+  const int C = P.C, Ts = P.Ts, WC = P.WC, Rq = P.Rq, TsP = 4 * WC;
+  uint32_t* tile = reinterpret_cast<uint32_t*>(smem);
+  uint8_t* ctrl = smem + (size_t)Rq * PW * 4;
+  uint32_t* xS = reinterpret_cast<uint32_t*>(ctrl);
+  uint32_t* xQ = xS + TsP;
+  uint4* chk = reinterpret_cast<uint4*>(xQ + TsP);
+  uint8_t* lo_b = reinterpret_cast<uint8_t*>(chk + WC);
+  uint8_t* hi_b = lo_b + TsP;
+  uint8_t* rr_b = hi_b + TsP;
+  uint64_t* bar = reinterpret_cast<uint64_t*>(rr_b + TsP);
+  volatile uint32_t* any_empty = reinterpret_cast<volatile uint32_t*>(bar + 1);
+
+  const int tid = threadIdx.x, nthreads = blockDim.x, lane = tid & 31;
+  const int j = (tid >> 5) * 8 + (lane & 7);          // word column of this thread
+  const int rg = lane >> 3;                           // row group 0..3
+  const uint32_t rank = cluster_ctarank(), ncta = cluster_nctarank();
+  const int c0 = (int)rank * Rq;                      // first channel of this CTA
+  const int nrows = max(0, min(Rq, C - c0));
+  const int ni = nrows > rg ? (nrows - rg + kFdRG - 1) / kFdRG : 0;   // rows rg + 4 i of this thread
+  const int wpc = (WC + (int)ncta - 1) / (int)ncta;   // word columns owned per CTA (F3)
+  const int nload = min(nrows, nthreads);
 
   if (tid == 0) {
-    mbar_init(&sm.bar, 1);
+    mbar_init(bar, nload > 0 ? nload : 1);
     fence_mbar_init();
-    for (int r = 0; r < P.m; ++r) { tma_prefetch_desc(&maps.src[r]); if (kExact) tma_prefetch_desc(&maps.dst[r]); }
+    *any_empty = 0;
   }
-  for (int i = tid; i < Ts; i += NT) { sm.dS[i] = 0; sm.dQ[i] = 0; sm.dcnt[i] = 0; }
   __syncthreads();
+  if (ncta > 1) cluster_sync_all();                   // peers' shared memory is live before any DSMEM access
 
   uint32_t phase = 0;
-  const int nbox = Rc / P.box_rows;
-  for (int64_t t = blockIdx.x; t < P.total_tiles; t += gridDim.x) {
+  const uint32_t nclusters = cluster_nid_x();
+  for (int64_t t = cluster_id_x(); t < P.total_tiles; t += nclusters) {
     const int b = (int)(t / P.tiles_per_beam);
     const int s0 = (int)(t % P.tiles_per_beam) * Ts;
-    // ------------------------------------------------------------------ F1: load the tile
-    if (tid == 0) {
-      mbar_arrive_expect_tx(&sm.bar, (uint32_t)(C * PW * 4));
-      for (int r = 0; r < P.m; ++r)
-        for (int bx = 0; bx < nbox; ++bx) {
-          const int row0 = r * Rc + bx * P.box_rows;
-          // kExact: off[r] == 0.  Otherwise x = s0 addresses byte s0 - off[r] of the row (never before the
-          // row's 16-byte aligned tensor origin) and the box is 16 bytes wider than the tile.
-          tma_load_2d(tile + (size_t)row0 * PW, &maps.src[r], s0, b * Rc + bx * P.box_rows, &sm.bar);
-        }
+    const int tw = min(Ts, P.S - s0);                 // valid columns of this tile
+    const uint8_t* gsrc = P.src + ((int64_t)b * C + c0) * P.stride + s0;   // row 0 of this CTA, column s0
+    // ------------------------------------------------------------------ F1: load the CTA's rows
+    if (nload == 0) {
+      if (tid == 0) mbar_arrive(bar);
+    } else if (tid < nload) {
+      uint32_t bytes = 0;
+      for (int r = tid; r < nrows; r += nthreads) {
+        const uint8_t* g = gsrc + (int64_t)r * P.stride;
+        const uint32_t off = (uint32_t)(reinterpret_cast<uintptr_t>(g) & 15);
+        bytes += (off + (uint32_t)tw + 15u) & ~15u;
+      }
+      mbar_arrive_expect_tx(bar, bytes);
+      for (int r = tid; r < nrows; r += nthreads) {
+        const uint8_t* g = gsrc + (int64_t)r * P.stride;
+        const uint32_t off = (uint32_t)(reinterpret_cast<uintptr_t>(g) & 15);
+        bulk_load(tile + (size_t)r * PW, g - off, (off + (uint32_t)tw + 15u) & ~15u, bar);
+      }
     }
-    mbar_wait(&sm.bar, phase);
+    mbar_wait(bar, phase);
     phase ^= 1;
 
+    // word offset of column s0 inside the shared-memory rows of this thread (same for all its rows)
+    const int offw = (int)((reinterpret_cast<uintptr_t>(gsrc + (int64_t)rg * P.stride) & 15) >> 2);
+    uint32_t* const col0 = tile + (size_t)rg * PW + offw + j;
+
     // ------------------------------------------------------------------ F2: column statistics
-    uint32_t S4[4] = {0, 0, 0, 0}, Q4[4] = {0, 0, 0, 0};
-    for (int cls = 0; cls < P.m; ++cls) {
-      const uint32_t* col = tile + (size_t)(cls * Rc + rg) * PW + wofs(cls) + wc;
-      int k = 0;
+    {
+      uint32_t S4[4] = {0, 0, 0, 0}, Q4[4] = {0, 0, 0, 0};
+      const uint32_t* col = col0;
+      int i = 0;
 #pragma unroll 2
-      for (; k + 4 <= nk; k += 4) {
-        const uint32_t a = col[(size_t)(k + 0) * RG * PW], bb = col[(size_t)(k + 1) * RG * PW];
-        const uint32_t c = col[(size_t)(k + 2) * RG * PW], d = col[(size_t)(k + 3) * RG * PW];
+      for (; i + 4 <= ni; i += 4, col += 16 * PW) {
+        const uint32_t a = col[0], bb = col[4 * PW], c = col[8 * PW], d = col[12 * PW];
         const uint32_t ab_lo = prmt_b32(a, bb, 0x5140u), ab_hi = prmt_b32(a, bb, 0x7362u);
         const uint32_t cd_lo = prmt_b32(c, d, 0x5140u), cd_hi = prmt_b32(c, d, 0x7362u);
         const uint32_t t0 = prmt_b32(ab_lo, cd_lo, 0x5410u), t1 = prmt_b32(ab_lo, cd_lo, 0x7632u);
@@ -186,168 +232,202 @@ __global__ void __launch_bounds__(4 * Ts) fd_u8_tile_kernel(const __grid_constan
         S4[2] = __dp4a(t2, 0x01010101u, S4[2]); Q4[2] = __dp4a(t2, t2, Q4[2]);
         S4[3] = __dp4a(t3, 0x01010101u, S4[3]); Q4[3] = __dp4a(t3, t3, Q4[3]);
       }
-      for (; k < nk; ++k) {
-        const uint32_t w = col[(size_t)k * RG * PW];
+      for (; i < ni; ++i, col += 4 * PW) {
+        const uint32_t w = col[0];
 #pragma unroll
-        for (int j = 0; j < 4; ++j) {
-          const uint32_t x = (w >> (8 * j)) & 0xffu;
-          S4[j] += x; Q4[j] += x * x;
+        for (int u = 0; u < 4; ++u) {
+          const uint32_t x = (w >> (8 * u)) & 0xffu;
+          S4[u] += x; Q4[u] += x * x;
         }
       }
-    }
-    {
-      uint32_t* r = sm.red + (size_t)(rg * WC + wc) * 8;
 #pragma unroll
-      for (int j = 0; j < 4; ++j) { r[j] = S4[j]; r[4 + j] = Q4[j]; }
-    }
-    __syncthreads();
-    // thread t < Ts owns column t: its S and Q live in registers across the iterations
-    uint32_t colS = 0, colQ = 0;
-    if (tid < Ts) {
-      const int cw = tid >> 2, cj = tid & 3;
-#pragma unroll
-      for (int g = 0; g < RG; ++g) {
-        colS += sm.red[(size_t)(g * WC + cw) * 8 + cj];
-        colQ += sm.red[(size_t)(g * WC + cw) * 8 + 4 + cj];
+      for (int u = 0; u < 4; ++u) {                    // reduce over the four row groups of the warp
+        S4[u] += __shfl_xor_sync(FULL, S4[u], 8);  Q4[u] += __shfl_xor_sync(FULL, Q4[u], 8);
+        S4[u] += __shfl_xor_sync(FULL, S4[u], 16); Q4[u] += __shfl_xor_sync(FULL, Q4[u], 16);
+      }
+      if (rg == 0) {
+        reinterpret_cast<uint4*>(xS)[j] = make_uint4(S4[0], S4[1], S4[2], S4[3]);
+        reinterpret_cast<uint4*>(xQ)[j] = make_uint4(Q4[0], Q4[1], Q4[2], Q4[3]);
       }
     }
+    if (ncta > 1) cluster_sync_all(); else __syncthreads();
 
     // ------------------------------------------------------------------ F3..F5: thresholds, on chip
+    // column ownership: CTA q owns word columns [q*wpc, (q+1)*wpc); thread tid < 4*wpc owns one column
+    const int ocol = (int)rank * wpc * 4 + tid;
+    const bool owner = tid < 4 * wpc && ocol < TsP;
+    uint32_t colS = 0, colQ = 0;
+    if (owner) {
+      if (ncta > 1) {
+        for (uint32_t q = 0; q < ncta; ++q) {
+          colS += dsmem_ld_u32(dsmem_addr(&xS[ocol], q));
+          colQ += dsmem_ld_u32(dsmem_addr(&xQ[ocol], q));
+        }
+      } else {
+        colS = xS[ocol];
+        colQ = xQ[ocol];
+      }
+    }
+    const uint32_t orank = ncta > 1 ? (uint32_t)(j / wpc) : 0u;   // CTA that publishes this thread's bounds
+
     for (int it = 0; it < P.n_thr; ++it) {
-      if (tid == 0) sm.any_cut = 0;
-      __syncthreads();
-      if (tid < Ts) {
-        int lo, hi;
-        const uint64_t V = (uint64_t)C * colQ - (uint64_t)colS * colS;
-        const U8Cut cut = make_cut_u8((uint32_t)C, colS, V, P.p[it]);
-        thread_bounds_u8_fast(cut, P.pf[it], V, lo, hi);
-        // Columns past the end of the row (last tile) are inert.  TMA checks the inner bound in 16-byte
-        // units (measured), so they may hold the next row's first bytes rather than zeros.
-        if (s0 + tid >= P.S) { lo = 0; hi = 255; }
-        const uint32_t r = rounded_mean_u8((uint32_t)C, colS);
-        reinterpret_cast<uint8_t*>(sm.lo4)[tid] = (uint8_t)lo;
-        reinterpret_cast<uint8_t*>(sm.hi4)[tid] = (uint8_t)hi;
-        reinterpret_cast<uint8_t*>(sm.r4)[tid] = (uint8_t)r;
-        if (!(lo == 0 && hi == 255)) sm.any_cut = 1;
+      if (owner) {
+        int lo = 0, hi = 255;
+        uint32_t r = 0;
+        if (ocol < tw) {
+          const uint64_t V = (uint64_t)C * colQ - (uint64_t)colS * colS;
+          const U8Cut cut = make_cut_u8((uint32_t)C, colS, V, P.p[it]);
+          thread_bounds_u8_fast(cut, P.pf[it], V, lo, hi);
+          r = rounded_mean_u8((uint32_t)C, colS);
+        }
+        lo_b[ocol] = (uint8_t)lo;
+        hi_b[ocol] = (uint8_t)hi;
+        rr_b[ocol] = (uint8_t)r;
+        uint16_t* c16 = reinterpret_cast<uint16_t*>(chk + (ocol >> 2));
+        const int u = ocol & 3, slot = (u & 1) * 2 + (u >> 1);       // E.lo, O.lo, E.hi, O.hi
+        c16[slot] = (uint16_t)((0x10000u - ((uint32_t)lo << 8)) & 0xffffu);
+        c16[4 + slot] = (uint16_t)(lo > hi ? 0u : ((((uint32_t)(hi - lo)) << 8) | 0xffu));
       }
-      __syncthreads();
-      if (sm.any_cut == 0) continue;                               // uniform: nothing can be cut in this tile
-      // F4a: packed range check, per-column bounds in the u16 lanes
-      const uint32_t lo4 = sm.lo4[wc], hi4 = sm.hi4[wc], r4 = sm.r4[wc];
-      uint32_t lob[4], hib[4];
-#pragma unroll
-      for (int j = 0; j < 4; ++j) { lob[j] = (lo4 >> (8 * j)) & 0xffu; hib[j] = (hi4 >> (8 * j)) & 0xffu; }
-      // odd chain: bytes 1 and 3 are the high bytes of the u16 lanes of w; even chain: bytes 0, 2 of w << 8
-      auto neg16 = [](uint32_t lo) { return (0x10000u - (lo << 8)) & 0xffffu; };
-      auto thr16 = [](uint32_t lo, uint32_t hi) { return lo > hi ? 0u : (((hi - lo) << 8) | 0xffu); };
-      auto ini16 = [](uint32_t lo, uint32_t hi) { return lo > hi ? 1u : 0u; };   // empty interval: always a hit
-      const uint32_t negO = neg16(lob[1]) | (neg16(lob[3]) << 16), negE = neg16(lob[0]) | (neg16(lob[2]) << 16);
-      const uint32_t thrO = thr16(lob[1], hib[1]) | (thr16(lob[3], hib[3]) << 16);
-      const uint32_t thrE = thr16(lob[0], hib[0]) | (thr16(lob[2], hib[2]) << 16);
-      const uint32_t iniO = ini16(lob[1], hib[1]) | (ini16(lob[3], hib[3]) << 16);
-      const uint32_t iniE = ini16(lob[0], hib[0]) | (ini16(lob[2], hib[2]) << 16);
-      const uint32_t chiE = (0x7fffu - hib[0]) | ((0x7fffu - hib[2]) << 16), cloE = (0x8000u - lob[0]) | ((0x8000u - lob[2]) << 16);
-      const uint32_t chiO = (0x7fffu - hib[1]) | ((0x7fffu - hib[3]) << 16), cloO = (0x8000u - lob[1]) | ((0x8000u - lob[3]) << 16);
-      const bool last = (it == P.n_thr - 1);
-      const bool need_stats = !last;
-      const bool need_cnt = P.counts != nullptr;
+      if (ncta > 1) cluster_sync_all(); else __syncthreads();
 
-      for (int cls = 0; cls < P.m; ++cls) {
-        uint32_t* col = tile + (size_t)(cls * Rc + rg) * PW + wofs(cls) + wc;
-        // F4b: exact fix of one word (rare path)
-        auto fix_word = [&](int k, uint32_t w) {
-          const uint32_t msk = bytes_outside_cols(w, chiE, cloE, chiO, cloO);
-          if (msk == 0) return;
-          col[(size_t)k * RG * PW] = (w & ~msk) | (r4 & msk);
+      // this thread's word column: packed constants and byte bounds, pulled from the publishing CTA
+      uint4 ck;
+      uint32_t lo4, hi4, r4;
+      if (ncta > 1) {
+        ck = dsmem_ld_u128(dsmem_addr(&chk[j], orank));
+        lo4 = dsmem_ld_u32(dsmem_addr(lo_b + 4 * j, orank));
+        hi4 = dsmem_ld_u32(dsmem_addr(hi_b + 4 * j, orank));
+        r4 = dsmem_ld_u32(dsmem_addr(rr_b + 4 * j, orank));
+      } else {
+        ck = chk[j];
+        lo4 = reinterpret_cast<const uint32_t*>(lo_b)[j];
+        hi4 = reinterpret_cast<const uint32_t*>(hi_b)[j];
+        r4 = reinterpret_cast<const uint32_t*>(rr_b)[j];
+      }
+      const uint32_t negE = ck.x, negO = ck.y, thrE = ck.z, thrO = ck.w;
+      const uint32_t chiE = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4240u), cloE = 0x80008000u - prmt_b32(lo4, 0u, 0x4240u);
+      const uint32_t chiO = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4341u), cloO = 0x80008000u - prmt_b32(lo4, 0u, 0x4341u);
+      // a column with an empty kept interval (lo > hi) cuts every value: no packed test can say that,
+      // so such a thread takes the exact path for all its words
+      const bool slow = __vcmpgtu4(lo4, hi4) != 0u;
+      const bool need_stats = it + 1 < P.n_thr;
+
+      uint32_t cnt4 = 0, sxE = 0, sxO = 0, sq[4] = {0, 0, 0, 0};   // per-column deltas of this thread, packed
+      auto fix_word = [&](uint32_t* ptr, uint32_t w, int i) {
+        const uint32_t m = bytes_outside_cols(w, chiE, cloE, chiO, cloO);
+        if (m == 0) return;
+        *ptr = (w & ~m) | (r4 & m);
+        const uint32_t f = w & m;
+        cnt4 += m & 0x01010101u;
+        sxE += prmt_b32(f, 0u, 0x4240u);
+        sxO += prmt_b32(f, 0u, 0x4341u);
+        sq[0] = __dp4a(f & 0x000000ffu, f, sq[0]);
+        sq[1] = __dp4a(f & 0x0000ff00u, f, sq[1]);
+        sq[2] = __dp4a(f & 0x00ff0000u, f, sq[2]);
+        sq[3] = __dp4a(f & 0xff000000u, f, sq[3]);
+        if (P.flags) {
+          uint8_t* fl = P.flags + ((int64_t)b * C + c0 + rg + kFdRG * i) * P.S + s0 + 4 * j;
 #pragma unroll
-          for (int j = 0; j < 4; ++j) {
-            if ((msk >> (8 * j)) & 1u) {
-              const uint32_t x = (w >> (8 * j)) & 0xffu, r = (r4 >> (8 * j)) & 0xffu;
-              const int colj = wc * 4 + j;
-              if (need_stats) {
-                atomicAdd(&sm.dS[colj], r - x);
-                atomicAdd(&sm.dQ[colj], r * r - x * x);
-              }
-              if (need_cnt) atomicAdd(&sm.dcnt[colj], 1u);
-              if (P.flags) {
-                const int ch = (rg + k * RG) * P.m + cls;          // row g of class cls is channel g*m + cls
-                P.flags[((int64_t)b * C + ch) * P.S + s0 + colj] = 1;
-              }
+          for (int u = 0; u < 4; ++u)
+            if ((m >> (8 * u)) & 1u) fl[u] = 1;
+        }
+      };
+      {
+        uint32_t* col = col0;
+        int i = 0;
+#pragma unroll 2
+        for (; i + 4 <= ni; i += 4, col += 16 * PW) {
+          const uint32_t w0 = col[0], w1 = col[4 * PW], w2 = col[8 * PW], w3 = col[12 * PW];
+          uint32_t aO = __viaddmax_u16x2(w0, negO, 0u), aE = __viaddmax_u16x2(w0 << 8, negE, 0u);
+          uint32_t bO = __viaddmax_u16x2(w1, negO, 0u), bE = __viaddmax_u16x2(w1 << 8, negE, 0u);
+          aO = __viaddmax_u16x2(w2, negO, aO); aE = __viaddmax_u16x2(w2 << 8, negE, aE);
+          bO = __viaddmax_u16x2(w3, negO, bO); bE = __viaddmax_u16x2(w3 << 8, negE, bE);
+          aO = __vmaxu2(aO, bO); aE = __vmaxu2(aE, bE);
+          if (slow || __vmaxu2(aO, thrO) != thrO || __vmaxu2(aE, thrE) != thrE) {
+            fix_word(col, w0, i);
+            fix_word(col + 4 * PW, w1, i + 1);
+            fix_word(col + 8 * PW, w2, i + 2);
+            fix_word(col + 12 * PW, w3, i + 3);
+          }
+        }
+        for (; i < ni; ++i, col += 4 * PW) fix_word(col, col[0], i);
+      }
+
+      if (need_stats || P.counts) {
+        uint32_t dS[4], dQ[4], cnt = 0;
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          const uint32_t c = (cnt4 >> (8 * u)) & 0xffu, r = (r4 >> (8 * u)) & 0xffu;
+          const uint32_t sx = ((u & 1) ? sxO : sxE) >> (16 * (u >> 1)) & 0xffffu;
+          dS[u] = c * r - sx;                        // modulo 2^32: the column totals stay below 2^32
+          dQ[u] = c * r * r - sq[u];
+          cnt += c;
+        }
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {
+          dS[u] += __shfl_xor_sync(FULL, dS[u], 8);  dQ[u] += __shfl_xor_sync(FULL, dQ[u], 8);
+          dS[u] += __shfl_xor_sync(FULL, dS[u], 16); dQ[u] += __shfl_xor_sync(FULL, dQ[u], 16);
+        }
+        if (need_stats && rg == 0) {
+          reinterpret_cast<uint4*>(xS)[j] = make_uint4(dS[0], dS[1], dS[2], dS[3]);
+          reinterpret_cast<uint4*>(xQ)[j] = make_uint4(dQ[0], dQ[1], dQ[2], dQ[3]);
+        }
+        if (P.counts) {
+          cnt = __reduce_add_sync(FULL, cnt);
+          if (lane == 0 && cnt) atomicAdd(&P.counts[it], (unsigned long long)cnt);
+        }
+      }
+      if (need_stats) {
+        if (ncta > 1) cluster_sync_all(); else __syncthreads();
+        if (owner) {
+          if (ncta > 1) {
+            for (uint32_t q = 0; q < ncta; ++q) {
+              colS += dsmem_ld_u32(dsmem_addr(&xS[ocol], q));
+              colQ += dsmem_ld_u32(dsmem_addr(&xQ[ocol], q));
             }
-          }
-        };
-        int k = 0;
-        for (; k + 8 <= nk; k += 8) {
-          uint32_t w[8];
-#pragma unroll
-          for (int u = 0; u < 8; ++u) w[u] = col[(size_t)(k + u) * RG * PW];
-          uint32_t accO = iniO, accE = iniE;
-#pragma unroll
-          for (int u = 0; u < 8; ++u) {
-            accO = __viaddmax_u16x2(w[u], negO, accO);
-            accE = __viaddmax_u16x2(w[u] << 8, negE, accE);
-          }
-          if (__vmaxu2(accO, thrO) != thrO || __vmaxu2(accE, thrE) != thrE) {
-#pragma unroll
-            for (int u = 0; u < 8; ++u) fix_word(k + u, w[u]);
-          }
-        }
-        for (; k < nk; ++k) fix_word(k, col[(size_t)k * RG * PW]);
-      }
-      __syncthreads();
-      if (tid < Ts && (need_stats || need_cnt)) {
-        if (need_stats) {
-          colS += sm.dS[tid];
-          colQ += sm.dQ[tid];
-          sm.dS[tid] = 0;
-          sm.dQ[tid] = 0;
-        }
-        if (need_cnt) {
-          const uint32_t cnt = sm.dcnt[tid];
-          sm.dcnt[tid] = 0;
-          if (cnt) atomicAdd(&P.counts[it], (unsigned long long)cnt);
-        }
-      }
-    }
-
-    // ------------------------------------------------------------------ F6: store the tile
-    if (kExact && s0 + Ts <= P.S) {                                 // (a ragged last tile is stored by the lanes:
-      fence_proxy_async_smem();                                     //  TMA stores clip in 16-byte units, measured)
-      __syncthreads();
-      if (tid == 0) {
-        for (int r = 0; r < P.m; ++r)
-          for (int bx = 0; bx < nbox; ++bx) {
-            const int row0 = r * Rc + bx * P.box_rows;
-            tma_store_2d(&maps.dst[r], s0, b * Rc + bx * P.box_rows, tile + (size_t)row0 * PW);
-          }
-        bulk_commit();
-        bulk_wait_read<0>();                                        // the tile may be overwritten after this
-      }
-      __syncthreads();
-    } else {
-      __syncthreads();
-      const int s = s0 + wc * 4;                                    // first sample of this thread's word column
-      if (s < P.S) {
-        const bool whole = s + 4 <= P.S;
-        for (int cls = 0; cls < P.m; ++cls) {
-          const uint32_t* col = tile + (size_t)(cls * Rc + rg) * PW + wofs(cls) + wc;
-          uint8_t* g = P.dst + ((int64_t)b * C + (int64_t)rg * P.m + cls) * P.stride + s;
-          const int64_t gstep = (int64_t)RG * P.m * P.stride;
-          if (whole) {
-#pragma unroll 4
-            for (int k = 0; k < nk; ++k) *reinterpret_cast<uint32_t*>(g + k * gstep) = col[(size_t)k * RG * PW];
           } else {
-            for (int k = 0; k < nk; ++k) {
-              const uint32_t w = col[(size_t)k * RG * PW];
-              for (int j = 0; s + j < P.S; ++j) g[k * gstep + j] = (uint8_t)(w >> (8 * j));
-            }
+            colS += xS[ocol];
+            colQ += xQ[ocol];
           }
         }
       }
-      __syncthreads();                                              // the tile may be overwritten after this
     }
+
+    // ------------------------------------------------------------------ F6: store the CTA's rows
+    fence_proxy_async_smem();                       // generic-proxy writes of the fix path -> async proxy
+    __syncthreads();
+    {
+      uint8_t* gdst = P.dst + ((int64_t)b * C + c0) * P.stride + s0;
+      bool issued = false;
+      for (int r = tid; r < nrows; r += nthreads) {
+        const uint32_t off = (uint32_t)(reinterpret_cast<uintptr_t>(gsrc + (int64_t)r * P.stride) & 15);
+        const uint8_t* srow = reinterpret_cast<const uint8_t*>(tile + (size_t)r * PW) + off;   // column s0
+        uint8_t* gd = gdst + (int64_t)r * P.stride;
+        // src and dst share their 16-byte phase (checked by the host), so the aligned interior of the
+        // destination is aligned in shared memory too
+        int h = (int)((16u - off) & 15u);
+        if (h > tw) h = tw;
+        const int body = (tw - h) & ~15;
+        if (body > 0) {
+          bulk_store(gd + h, srow + h, (uint32_t)body);
+          issued = true;
+        }
+        int i = 0;
+        for (; i + 4 <= h; i += 4) *reinterpret_cast<uint32_t*>(gd + i) = *reinterpret_cast<const uint32_t*>(srow + i);
+        for (; i < h; ++i) gd[i] = srow[i];
+        i = h + body;
+        for (; i + 4 <= tw; i += 4) *reinterpret_cast<uint32_t*>(gd + i) = *reinterpret_cast<const uint32_t*>(srow + i);
+        for (; i < tw; ++i) gd[i] = srow[i];
+      }
+      if (issued) {
+        bulk_commit();
+        bulk_wait_read<0>();                        // the rows may be overwritten after this
+      }
+    }
+    __syncthreads();
   }
-  if (kExact && tid == 0) bulk_wait_all<0>();
+  bulk_wait_all<0>();
+  if (ncta > 1) cluster_sync_all();                 // no CTA leaves while a peer may still read its shared memory
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -70,7 +70,7 @@ int validate(int op, void* data, int beams, int channels, int samples, rfim_dtyp
   if (z.reserved != 0) return RFIM_ERR_INVALID;
   if (z.sample_stride != 0 && z.sample_stride < samples) return RFIM_ERR_INVALID;
   if (z.window < 0 || z.bin_size < 0) return RFIM_ERR_INVALID;
-  if (z.variant < 0 || z.variant > 4) return RFIM_ERR_INVALID;
+  if (z.variant < 0 || z.variant > 8) return RFIM_ERR_INVALID;
   if (op == 1 && z.bin_size != 0) {
     if (z.bin_size > channels || channels % z.bin_size != 0) return RFIM_ERR_INVALID;
     if (dtype == RFIM_U8 && z.bin_size != channels && z.bin_size > 65536) return RFIM_ERR_INVALID;
@@ -190,113 +190,78 @@ int launch_td_u8(const Call& c) {
 }
 
 // ------------------------------------------------------------------------------------------ FD u8
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
-                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
-                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+// Geometry of the cluster kernel for the request, or false when only the generic kernel can run it.
+struct FdPlan { int cl, pw, ts, wc, rq, tiles_per_beam, smem; };
 
-EncodeTiledFn encode_tiled_fn() {
-  static EncodeTiledFn fn = [] {
-    void* p = nullptr;
-    cudaDriverEntryPointQueryResult q;
-    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
-        q != cudaDriverEntryPointSuccess)
-      p = nullptr;
-    return reinterpret_cast<EncodeTiledFn>(p);
-  }();
-  return fn;
-}
+constexpr int kFdPw[] = {136, 120, 104, 88, 72, 56, 40, 24};    // row pitches (words), PW mod 32 in {8, 24}
 
-struct FdPlan { int ts, m, rows_per_class, box_rows, smem; bool exact; };
-
-template <int Ts, bool kExact>
-size_t fd_smem_bytes(int C) {
-  const size_t row_bytes = kExact ? Ts : Ts + 16;
-  return (((size_t)C * row_bytes + 127) & ~(size_t)127) + sizeof(rfim::FdSmem<Ts>);
-}
-size_t fd_smem_for(int ts, int C) {
-  switch (ts) {
-    case 128: return fd_smem_bytes<128, true>(C);
-    case 64: return fd_smem_bytes<64, true>(C);
-    case 32: return fd_smem_bytes<32, true>(C);
-    case 112: return fd_smem_bytes<112, false>(C);
-    default: return fd_smem_bytes<48, false>(C);
+bool plan_fd_u8_for(const Call& c, int cl, size_t budget, FdPlan& pl) {
+  const int rq = (c.channels + cl - 1) / cl;
+  if (rq > 1020) return false;                                   // packed per-thread delta counters (255 rows/thread)
+  for (int pw : kFdPw) {
+    int ts_max = 4 * pw - 16;
+    if (ts_max > 512) ts_max = 512;                              // 4 * WC <= 512 threads
+    const int tiles = (c.samples + ts_max - 1) / ts_max;
+    int ts = (c.samples + tiles - 1) / tiles;
+    ts = (ts + 3) & ~3;
+    const int wc = ((ts / 4) + 7) & ~7;
+    const size_t smem = rfim::fd_cluster_smem_bytes(pw, rq, wc);
+    if (smem > budget) continue;
+    pl.cl = cl; pl.pw = pw; pl.ts = ts; pl.wc = wc; pl.rq = rq; pl.tiles_per_beam = tiles; pl.smem = (int)smem;
+    return true;
   }
+  return false;
 }
 
-// Tile geometry for the request, or false when only the generic kernel can run it.  `big` prefers the
-// widest tile that fits one CTA per SM over a narrower one with two CTAs per SM (variant 3).
-bool plan_fd_u8_tile(const Call& c, bool big, FdPlan& pl) {
+bool plan_fd_u8_cluster(const Call& c, int force_cl, FdPlan& pl) {
   if (c.policy != RFIM_REPLACE_MEAN || c.bin_size != c.channels) return false;
-  int m = 1;
-  while ((((int64_t)m * c.stride) & 15) != 0) m <<= 1;       // rows per 16-byte alignment period
-  if (m > rfim::kFdMaxClasses || c.channels % m != 0) return false;
-  if (c.channels > 60000) return false;                      // 32-bit column totals inside the kernel
   const uintptr_t src = reinterpret_cast<uintptr_t>(c.data), dst = reinterpret_cast<uintptr_t>(c.out);
-  pl.exact = (m == 1) && ((src | dst) & 15) == 0;
-  if (!pl.exact && ((src | dst) & 3) != 0) return false;     // 32-bit stores of the tile
-  pl.m = m;
-  pl.rows_per_class = c.channels / m;
-  static const int exact_ts[3] = {128, 64, 32}, over_ts[2] = {112, 48};
-  const int* cand = pl.exact ? exact_ts : over_ts;
-  const int ncand = pl.exact ? 3 : 2;
-  const size_t half = (size_t)(kMaxSmem + 1024) / 2 - 1024;  // two CTAs per SM (1 KB reserved per CTA)
-  // TMA boxes: rows per box divides the class, <= 256, and every box lands 128-byte aligned in shared memory
-  auto boxes_for = [&](int ts) {
-    const int row_bytes = pl.exact ? ts : ts + 16;
-    if (m > 1 && ((int64_t)pl.rows_per_class * row_bytes) % 128 != 0) return 0;
-    int best = 0;
-    for (int d = 1; d <= 256 && d <= pl.rows_per_class; ++d)
-      if (pl.rows_per_class % d == 0 && (d * row_bytes) % 128 == 0) best = d;
-    if (pl.rows_per_class == best) return best;                // a single box needs no alignment of its size
-    if (best == 0 && pl.rows_per_class <= 256) return pl.rows_per_class;
-    return (best && pl.rows_per_class / best <= 64) ? best : 0;
-  };
-  pl.ts = 0;
-  for (int pass = big ? 1 : 0; pass < 2 && !pl.ts; ++pass)
-    for (int i = 0; i < ncand && !pl.ts; ++i)
-      if (fd_smem_for(cand[i], c.channels) <= (pass == 0 ? half : (size_t)kMaxSmem) && boxes_for(cand[i]) > 0)
-        pl.ts = cand[i];
-  if (!pl.ts) return false;
-  pl.box_rows = boxes_for(pl.ts);
-  pl.smem = (int)fd_smem_for(pl.ts, c.channels);
-  return true;
-}
-
-// one 2-D tensor per alignment class r: rows r, r+m, r+2m, ... of the [beams*channels][pitch] matrix,
-// origin rounded down to 16 bytes (off[r] bytes before the row start)
-bool encode_fd_maps(const Call& c, const FdPlan& pl, uint8_t* base, CUtensorMap* maps, int* off) {
-  EncodeTiledFn enc = encode_tiled_fn();
-  if (!enc) return false;
-  for (int r = 0; r < pl.m; ++r) {
-    const uintptr_t addr = reinterpret_cast<uintptr_t>(base) + (uintptr_t)r * (uintptr_t)c.stride;
-    off[r] = (int)(addr & 15);
-    cuuint64_t dims[2] = {(cuuint64_t)c.samples + (cuuint64_t)off[r],
-                          (cuuint64_t)c.beams * (cuuint64_t)pl.rows_per_class};
-    cuuint64_t strides[1] = {(cuuint64_t)pl.m * (cuuint64_t)c.stride};
-    cuuint32_t box[2] = {(cuuint32_t)(pl.exact ? pl.ts : pl.ts + 16), (cuuint32_t)pl.box_rows};
-    cuuint32_t estr[2] = {1, 1};
-    if (enc(&maps[r], CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, reinterpret_cast<void*>(addr - off[r]), dims, strides, box,
-            estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
-            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-      return false;
+  if ((src & 3) != 0 || (c.stride & 3) != 0) return false;       // 32-bit word columns
+  if (((src ^ dst) & 15) != 0) return false;                     // aligned interiors of src and dst rows coincide
+  if (c.channels > 60000) return false;                          // 32-bit column totals inside the kernel
+  const size_t half = (size_t)(kMaxSmem + 1024) / 2 - 1024;      // two CTAs per SM (1 KB reserved per CTA)
+  if (force_cl) return plan_fd_u8_for(c, force_cl, half, pl) || plan_fd_u8_for(c, force_cl, (size_t)kMaxSmem, pl);
+  // smallest cluster that still gets the widest tile with two CTAs per SM; else the widest tile any cluster gets
+  FdPlan best; bool have = false;
+  for (int cl = 1; cl <= 8; cl *= 2) {
+    FdPlan p;
+    if (!plan_fd_u8_for(c, cl, half, p)) continue;
+    if (!have || p.ts > best.ts) { best = p; have = true; }
+    if (p.pw == kFdPw[0]) break;
   }
-  return true;
+  if (!have) {
+    for (int cl = 8; cl >= 1 && !have; cl /= 2) have = plan_fd_u8_for(c, cl, (size_t)kMaxSmem, best);
+  }
+  if (have) pl = best;
+  return have;
 }
 
-template <int Ts, bool kExact>
-int launch_fd_tile(const Call& c, const FdPlan& pl, const rfim::FdMaps& maps, rfim::FdU8Params& P, int sms,
-                   const char* name) {
-  auto kernel = rfim::fd_u8_tile_kernel<Ts, kExact>;
+template <int PW>
+int launch_fd_cluster(const Call& c, const FdPlan& pl, const rfim::FdU8Params& P, int sms) {
+  auto kernel = rfim::fd_u8_cluster_kernel<PW>;
   CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem));
-  int occ = 0;
-  CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, 4 * Ts, pl.smem));
-  if (occ < 1) occ = 1;
-  int64_t grid = P.total_tiles;
-  if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)pl.cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.blockDim = dim3((unsigned)(4 * pl.wc), 1, 1);
+  cfg.dynamicSmemBytes = (size_t)pl.smem;
+  cfg.stream = c.stream;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int nclusters = 0;
+  cfg.gridDim = dim3((unsigned)(sms * 2 / pl.cl * pl.cl), 1, 1);
+  CUDA_TRY(cudaOccupancyMaxActiveClusters(&nclusters, kernel, &cfg));
+  if (nclusters < 1) return RFIM_ERR_UNSUPPORTED;
+  int64_t want = P.total_tiles;
+  if (want > nclusters) want = nclusters;
+  cfg.gridDim = dim3((unsigned)(want * pl.cl), 1, 1);
   int st = clear_outputs(c);
   if (st != RFIM_OK) return st;
-  kernel<<<(unsigned)grid, 4 * Ts, pl.smem, c.stream>>>(maps, P);
-  return after_launch(name);
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, kernel, P));
+  static const char* names[4] = {"fd_u8_cluster1", "fd_u8_cluster2", "fd_u8_cluster4", "fd_u8_cluster8"};
+  return after_launch(names[pl.cl == 1 ? 0 : pl.cl == 2 ? 1 : pl.cl == 4 ? 2 : 3]);
 }
 
 int launch_fd_u8(const Call& c) {
@@ -315,25 +280,25 @@ int launch_fd_u8(const Call& c) {
   if (st != RFIM_OK) return st;
 
   FdPlan pl;
-  bool can_tile = c.variant != 1 && plan_fd_u8_tile(c, c.reserved_team == 1, pl);
-  rfim::FdMaps maps;
-  if (can_tile) {
-    int off_dst[rfim::kFdMaxClasses] = {0, 0, 0, 0};
-    can_tile = encode_fd_maps(c, pl, static_cast<uint8_t*>(c.data), maps.src, P.off) &&
-               (!pl.exact || encode_fd_maps(c, pl, static_cast<uint8_t*>(c.out), maps.dst, off_dst));
-  }
-  if (c.variant == 2 && !can_tile) return RFIM_ERR_UNSUPPORTED;
-  if (can_tile) {
-    P.m = pl.m; P.rows_per_class = pl.rows_per_class; P.box_rows = pl.box_rows;
-    P.tiles_per_beam = (c.samples + pl.ts - 1) / pl.ts;
-    P.total_tiles = (int64_t)P.tiles_per_beam * c.beams;
-    switch (pl.ts) {
-      case 128: return launch_fd_tile<128, true>(c, pl, maps, P, dv.sms, "fd_u8_tile128");
-      case 64: return launch_fd_tile<64, true>(c, pl, maps, P, dv.sms, "fd_u8_tile64");
-      case 32: return launch_fd_tile<32, true>(c, pl, maps, P, dv.sms, "fd_u8_tile32");
-      case 112: return launch_fd_tile<112, false>(c, pl, maps, P, dv.sms, "fd_u8_tile112x");
-      default: return launch_fd_tile<48, false>(c, pl, maps, P, dv.sms, "fd_u8_tile48x");
+  int force_cl = 0;
+  if (c.variant >= 5 && c.variant <= 8) force_cl = 1 << (c.variant - 5);
+  const bool can_cluster = c.variant != 1 && plan_fd_u8_cluster(c, force_cl, pl);
+  if (c.variant >= 2 && !can_cluster) return RFIM_ERR_UNSUPPORTED;
+  if (can_cluster) {
+    P.Ts = pl.ts; P.WC = pl.wc; P.Rq = pl.rq;
+    P.tiles_per_beam = pl.tiles_per_beam;
+    P.total_tiles = (int64_t)pl.tiles_per_beam * c.beams;
+    switch (pl.pw) {
+      case 136: st = launch_fd_cluster<136>(c, pl, P, dv.sms); break;
+      case 120: st = launch_fd_cluster<120>(c, pl, P, dv.sms); break;
+      case 104: st = launch_fd_cluster<104>(c, pl, P, dv.sms); break;
+      case 88: st = launch_fd_cluster<88>(c, pl, P, dv.sms); break;
+      case 72: st = launch_fd_cluster<72>(c, pl, P, dv.sms); break;
+      case 56: st = launch_fd_cluster<56>(c, pl, P, dv.sms); break;
+      case 40: st = launch_fd_cluster<40>(c, pl, P, dv.sms); break;
+      default: st = launch_fd_cluster<24>(c, pl, P, dv.sms); break;
     }
+    if (st != RFIM_ERR_UNSUPPORTED || c.variant >= 2) return st;
   }
   if (c.policy != RFIM_REPLACE_MEAN || c.bin_size != c.channels) return RFIM_ERR_UNSUPPORTED;
   const int64_t ncol = (int64_t)c.beams * c.samples;

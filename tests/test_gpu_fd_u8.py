@@ -14,6 +14,7 @@ pytestmark = pytest.mark.gpu
 
 DEV = "cuda:0"
 TILE, GENERIC = rfim.VARIANT_STAGED, rfim.VARIANT_GENERIC
+CL1, CL2, CL4, CL8 = 5, 6, 7, 8          # rfim_opts.variant: force the cluster size of the FDSC kernel
 
 
 def run_gpu(x_np, ks, variant=rfim.VARIANT_AUTO, inplace=False, pitch=None, want_flags=True):
@@ -64,7 +65,7 @@ def test_config1_shape_fd(variant):
     cfg = synth.config(1)
     x = synth.fill_host(cfg)
     name, counts = check(x, [3.0], variant=variant)
-    assert name == ("fd_u8_tile128" if variant == TILE else "fd_u8_generic")
+    assert name == ("fd_u8_cluster1" if variant == TILE else "fd_u8_generic")
     _, flags, _ = oracle.freq_sigma_cut(x, [3.0])
     assert flags[0, 7].mean() > 0.9 and flags[0, 40].mean() > 0.9
 
@@ -77,7 +78,7 @@ def test_config3_arts_like_all_beams():
     synth.fill_device(cfg, x)
     x_np = x.cpu().numpy()
     name, counts = check(x_np, cfg["thresholds"], inplace=True)
-    assert name == "fd_u8_tile48x"
+    assert name == "fd_u8_cluster8"
     assert all(int(c) > 0 for c in counts)
     check(x_np[:1], cfg["thresholds"], variant=GENERIC)
 
@@ -100,8 +101,8 @@ def test_config4_chain_two_beams():
                                  (1536, 212), (2000, 96), (4096, 70), (7000, 33)])
 @pytest.mark.parametrize("variant", [rfim.VARIANT_AUTO, GENERIC])
 def test_shapes(C, S, variant):
-    """Row pitch S runs through every alignment class count (m = 1, 2, 4 and, for odd S, the generic path);
-    channel counts that are not multiples of the row groups; ragged last tile."""
+    """Row pitch S runs through every 16-byte phase pattern (S mod 16 = 0, 8, 4, 12; S not a multiple of 4 takes
+    the generic path); channel counts that are not multiples of the row groups or the cluster size; ragged tiles."""
     x = noisy((2, C, S), seed=C * 7 + S)
     if C >= 8:
         x[0, C // 2, :] = np.minimum(x[0, C // 2, :].astype(int) + 90, 255).astype(np.uint8)   # narrow-band RFI
@@ -109,11 +110,8 @@ def test_shapes(C, S, variant):
         x[1, C - 1, S - 1] = 0
         x[0, :, 0] = 77                                                                          # constant column
     name, _ = check(x, [4.0, 3.0], variant=variant)
-    m = 1
-    while (m * S) % 16:
-        m *= 2
-    tiled = variant != GENERIC and m <= 4 and C % m == 0 and C * (32 if m == 1 else 64) <= 220 * 1024
-    assert name.startswith("fd_u8_tile") == tiled, (name, m)
+    tiled = variant != GENERIC and S % 4 == 0
+    assert name.startswith("fd_u8_cluster") == tiled, name
     check(x, [3.25, 3.25, 3.25], variant=variant, inplace=True)
 
 
@@ -127,20 +125,21 @@ def test_padded_pitch(pitch):
 
 
 def test_misaligned_out():
-    """out 4 bytes off data's 16-byte phase: the over-read tile path stores with 32-bit words, so it still
-    runs; 1 byte off: only the generic kernel can."""
+    """out with another 16-byte phase than data: the aligned interiors of the rows do not coincide, so only the
+    generic kernel can run; a whole 16 bytes off is fine for the cluster kernel."""
     x = noisy((1, 16, 1000), seed=12)
     x[0, 3, :] = 250
     xd = torch.from_numpy(x).to(DEV)
     ref, _, _ = oracle.freq_sigma_cut(x, [3.0])
-    for shift, want in ((4, "fd_u8_tile112x"), (1, "fd_u8_generic")):
-        obuf = torch.zeros(16 * 1000 + 16, dtype=torch.uint8, device=DEV)
+    for shift, want in ((4, "fd_u8_generic"), (1, "fd_u8_generic"), (16, "fd_u8_cluster1")):
+        obuf = torch.zeros(16 * 1000 + 32, dtype=torch.uint8, device=DEV)
         out = obuf[shift:shift + 16000].view(1, 16, 1000)
         rfim.rfim_freq_sigma_cut(xd, [3.0], out=out)
         torch.cuda.synchronize()
         assert rfim.rfim_last_variant() == want
         assert np.array_equal(out.cpu().numpy(), ref)
         assert int(obuf[:shift].sum()) == 0 and int(obuf[shift + 16000:].sum()) == 0
+    out = obuf[4:4 + 16000].view(1, 16, 1000)
     with pytest.raises(rfim.RfimError) as e:
         rfim.rfim_freq_sigma_cut(xd, [3.0], out=out, variant=TILE)
     assert e.value.status == -2
@@ -155,7 +154,7 @@ def test_unaligned_base_pointer_tile_path():
     v.copy_(torch.from_numpy(x).to(DEV))
     rfim.rfim_freq_sigma_cut(v, [4.0, 3.0])
     torch.cuda.synchronize()
-    assert rfim.rfim_last_variant().startswith("fd_u8_tile")
+    assert rfim.rfim_last_variant().startswith("fd_u8_cluster")
     ref, _, _ = oracle.freq_sigma_cut(x, [4.0, 3.0])
     assert np.array_equal(v.cpu().numpy(), ref)
     assert int(buf[:4].sum()) == 0 and int(buf[4 + 2 * 32 * 500:].sum()) == 0
@@ -208,9 +207,11 @@ def test_many_tiles_grid_wraps():
     x = noisy((40, 64, 2100), seed=71)
     x[:, 9, ::5] = 255
     name, _ = check(x, [4.0, 3.0])
-    assert name == "fd_u8_tile112x"
-    name, _ = check(x[:, :, :2096], [4.0, 3.0])
-    assert name == "fd_u8_tile128"
+    assert name == "fd_u8_cluster1"
+    name, _ = check(np.ascontiguousarray(x[:, :, :2096]), [4.0, 3.0])
+    assert name == "fd_u8_cluster1"
+    for v in (CL2, CL4, CL8):
+        check(x[:13], [4.0, 3.0], variant=v)
 
 
 def test_no_flags_no_counts_other_stream():
@@ -239,3 +240,35 @@ def test_unsupported_requests_fail_loudly():
     with pytest.raises(rfim.RfimError) as e:
         rfim.rfim_freq_sigma_cut(x, [3.0], policy="median")
     assert e.value.status == -2
+
+
+# ------------------------------------------------------------------------ forced cluster sizes
+@pytest.mark.parametrize("variant,name", [(CL1, "fd_u8_cluster1"), (CL2, "fd_u8_cluster2"), (CL4, "fd_u8_cluster4"),
+                                          (CL8, "fd_u8_cluster8")])
+@pytest.mark.parametrize("C,S", [(3, 64), (8, 100), (37, 1000), (200, 520), (1000, 2100), (1536, 700)])
+def test_cluster_sizes(variant, name, C, S):
+    """Channels split over 1, 2, 4, 8 CTAs: uneven splits, CTAs without any channel (C < cluster size), several
+    tiles per beam with a ragged last one, partial sums and column deltas exchanged through DSMEM."""
+    x = noisy((3, C, S), seed=C + S)
+    if C > 1020 * (1 << (variant - CL1)):
+        # more than 1020 channels per CTA: the packed per-thread delta counters would overflow, so the
+        # library refuses the forced variant (auto picks a larger cluster)
+        with pytest.raises(rfim.RfimError) as e:
+            run_gpu(x, [4.0], variant=variant)
+        assert e.value.status == -2
+        return
+    x[0, C // 2, :] = np.minimum(x[0, C // 2, :].astype(int) + 90, 255).astype(np.uint8)
+    x[1, :, S // 3] = 3
+    x[2, C - 1, ::3] = 255
+    got, _ = check(x, [4.0, 3.0, 3.0], variant=variant)
+    assert got == name
+    check(x, [3.25, 3.25], variant=variant, inplace=True)
+
+
+def test_cluster_pitch_and_phase():
+    """Padded pitches with every 16-byte phase pattern, through the 8-CTA cluster."""
+    for pitch in (1008, 1004, 1012, 1024):
+        x = noisy((2, 100, 1000), seed=pitch)
+        x[:, 9, :] = 200
+        check(x, [4.0, 3.0], pitch=pitch, variant=CL8)
+        check(x, [4.0, 3.0], pitch=pitch, variant=CL4, inplace=True)
