@@ -189,6 +189,65 @@ int launch_td_u8(const Call& c) {
   return after_launch("td_u8_generic");
 }
 
+
+// ------------------------------------------------------------------------------------------ TD f32
+template <int kTW>
+int launch_td_f32_t(const Call& c, rfim::TdF32Params& P, bool stage, int sms, const char* name) {
+  const int nt = rfim::f32_teams<kTW>();
+  const size_t smem = (stage ? (((size_t)P.seg * 4 + 15) & ~(size_t)15) : 0) + (size_t)nt * sizeof(rfim::F32Team) + 16;
+  void (*kernel)(const rfim::TdF32Params) = stage ? rfim::td_f32_kernel<kTW, true> : rfim::td_f32_kernel<kTW, false>;
+  CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int occ = 0;
+  CUDA_TRY(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kernel, rfim::kF32Threads, smem));
+  if (occ < 1) return RFIM_ERR_UNSUPPORTED;
+  int64_t grid = P.rows * P.segs_per_row;
+  if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
+  int st = clear_outputs(c);
+  if (st != RFIM_OK) return st;
+  kernel<<<(unsigned)grid, rfim::kF32Threads, smem, c.stream>>>(P);
+  return after_launch(name);
+}
+
+int launch_td_f32(const Call& c) {
+  rfim::TdF32Params P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const float*>(c.data);
+  P.dst = static_cast<float*>(c.out);
+  P.rows = (int64_t)c.beams * c.channels;
+  P.stride = c.stride;
+  P.S = c.samples;
+  P.window = c.window;
+  P.n_thr = c.n_thr;
+  P.policy = (int)c.policy;
+  for (int i = 0; i < c.n_thr; ++i) P.k[i] = c.thr[i];
+  P.flags = c.flags;
+  P.counts = c.counts;
+  DevInfo dv;
+  int st = dev_info(dv);
+  if (st != RFIM_OK) return st;
+  // segment = run of whole windows staged in shared memory: the whole row when it fits beside the team
+  // scratch with three CTAs per SM, else the whole row alone, else as many windows as fit
+  const int overhead = 8 * (int)sizeof(rfim::F32Team) + 16;
+  const int cap3 = ((kMaxSmem + 1024) / 3 - 1024 - overhead) / 4;
+  const int cap1 = (kMaxSmem - overhead) / 4;
+  bool stage = c.variant != 1;
+  if (c.samples <= cap1) { P.seg = c.samples; P.segs_per_row = 1; }
+  else if (c.window <= cap1) {
+    const int cap = c.window <= cap3 ? cap3 : cap1;
+    P.seg = cap / c.window * c.window;
+    P.segs_per_row = (c.samples + P.seg - 1) / P.seg;
+  } else { stage = false; }
+  if (!stage) { P.seg = c.samples; P.segs_per_row = 1; }
+  if (c.variant == 2 && !stage) return RFIM_ERR_UNSUPPORTED;
+  const uintptr_t a = reinterpret_cast<uintptr_t>(c.data) | reinterpret_cast<uintptr_t>(c.out);
+  P.bulk = ((a & 15) == 0 && (c.stride % 4 == 0 || P.rows == 1) && (P.segs_per_row == 1 || P.seg % 4 == 0)) ? 1 : 0;
+  const int nwin = (P.seg + c.window - 1) / c.window;     // windows per (full) segment
+  if (nwin >= 6) return launch_td_f32_t<1>(c, P, stage, dv.sms, stage ? "td_f32_staged_w1" : "td_f32_global_w1");
+  if (nwin >= 3) return launch_td_f32_t<2>(c, P, stage, dv.sms, stage ? "td_f32_staged_w2" : "td_f32_global_w2");
+  if (nwin == 2) return launch_td_f32_t<4>(c, P, stage, dv.sms, stage ? "td_f32_staged_w4" : "td_f32_global_w4");
+  return launch_td_f32_t<8>(c, P, stage, dv.sms, stage ? "td_f32_staged_w8" : "td_f32_global_w8");
+}
+
 // ------------------------------------------------------------------------------------------ FD u8
 // Geometry of the cluster kernel for the request, or false when only the generic kernel can run it.
 struct FdPlan { int cl, pw, ts, wc, rq, tiles_per_beam, smem; };
@@ -325,7 +384,7 @@ int rfim_time_sigma_cut(void* data, int beams, int channels, int samples, rfim_d
     return copy_through(c);
   }
   if (dtype == RFIM_U8) return launch_td_u8(c);
-  return RFIM_ERR_UNSUPPORTED;
+  return launch_td_f32(c);
 }
 
 int rfim_freq_sigma_cut(void* data, int beams, int channels, int samples, rfim_dtype dtype,
