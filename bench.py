@@ -160,7 +160,7 @@ def run_ours(args, cfg):
     import torch
 
     import paper_2001_03389_b200 as rfim
-    from paper_2001_03389_b200 import synth
+    from paper_2001_03389_b200 import shard, synth
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -185,7 +185,7 @@ def run_ours(args, cfg):
     gen_chunk = 48
     for b0 in range(0, B, gen_chunk):                             # rank r holds beams [r*B, (r+1)*B) of the stream
         nb = min(gen_chunk, B - b0)
-        synth.fill_device(cfg, x[b0:b0 + nb], beam0=rank * B + b0, beams=nb)
+        synth.fill_device(cfg, x[b0:b0 + nb], beam0=shard.weak_scaling_beam0(B, rank) + b0, beams=nb)
     torch.cuda.synchronize()
 
     def step(evs=None):
@@ -222,10 +222,7 @@ def run_ours(args, cfg):
     rfim.rfim_freq_sigma_cut(y[:1], FD_KS); fd_name = rfim.rfim_last_variant()
     torch.cuda.synchronize()
     ms_total = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = shard.max_over_ranks(ms_total, dev)
     ms_step = ms_total / K
     td_ms = float(np.mean([e[0].elapsed_time(e[1]) for e in evs]))
     fd_ms = float(np.mean([e[1].elapsed_time(e[2]) for e in evs]))
