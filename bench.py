@@ -191,10 +191,10 @@ def run_ours(args, cfg):
     def step(evs=None):
         if evs:
             evs[0].record()
-        rfim.rfim_time_sigma_cut(x, TD_KS, out=y)
+        rfim.rfim_time_sigma_cut(x, TD_KS, out=y, variant=args.td_variant)
         if evs:
             evs[1].record()
-        rfim.rfim_freq_sigma_cut(y, FD_KS)
+        rfim.rfim_freq_sigma_cut(y, FD_KS, variant=args.fd_variant)
         if evs:
             evs[2].record()
 
@@ -340,6 +340,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--beams", type=int, default=0, help="override the beam count (testing only)")
+    ap.add_argument("--td-variant", type=int, default=0, help="kernel variant for TDSC (tuning only; 0 = auto)")
+    ap.add_argument("--fd-variant", type=int, default=0, help="kernel variant for FDSC (tuning only; 0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     args = ap.parse_args()

@@ -124,7 +124,7 @@ int after_launch(const char* name) {
 }
 
 // ------------------------------------------------------------------------------------------ TD u8
-struct StagedPlan { int nteams, team, slot_bytes, queue_entries, smem; };
+struct StagedPlan { int nteams, team, slot_bytes, sum_entries, smem; };
 
 bool plan_td_u8_staged(const Call& c, StagedPlan& pl) {
   if (c.window != c.samples || c.policy != RFIM_REPLACE_MEAN) return false;
@@ -132,9 +132,9 @@ bool plan_td_u8_staged(const Call& c, StagedPlan& pl) {
   if (((reinterpret_cast<uintptr_t>(c.data) ^ reinterpret_cast<uintptr_t>(c.out)) & 15) != 0) return false;
   if (c.samples > 65000) return false;                    // 32-bit S, Q totals inside the kernel
   pl.slot_bytes = (c.samples + 30 + 15) & ~15;
-  pl.queue_entries = ((pl.slot_bytes / 16) + 3) & ~3;
-  // per team: one slot, one hit queue, one control block; sixteen teams keep sixteen rows in flight
-  const int per_team = pl.slot_bytes + pl.queue_entries * 2 + rfim::kCtrlBytes;
+  pl.sum_entries = ((pl.slot_bytes / 16) + 15) & ~15;     // max byte and min byte per 16-byte group
+  // per team: one slot, its group summaries, one control block; sixteen teams keep sixteen rows in flight
+  const int per_team = pl.slot_bytes + pl.sum_entries * 2 + rfim::kCtrlBytes;
   pl.nteams = kMaxSmem / per_team;
   if (pl.nteams > 16) pl.nteams = 16;
   if (pl.nteams < 4) return false;
@@ -167,7 +167,7 @@ int launch_td_u8(const Call& c) {
   if (c.variant == 2 && !can_stage) return RFIM_ERR_UNSUPPORTED;
   if (can_stage && c.variant != 1) {
     P.slot_bytes = pl.slot_bytes;
-    P.queue_entries = pl.queue_entries;
+    P.sum_entries = pl.sum_entries;
     void (*kernel)(const rfim::TdU8Params);
     if (pl.team == 2) kernel = c.flags ? rfim::td_u8_staged_kernel<2, true> : rfim::td_u8_staged_kernel<2, false>;
     else kernel = c.flags ? rfim::td_u8_staged_kernel<1, true> : rfim::td_u8_staged_kernel<1, false>;

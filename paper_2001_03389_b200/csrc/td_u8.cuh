@@ -4,14 +4,16 @@
 //   td_u8_staged_kernel   the hot path.  One warp owns one
 //       (beam, channel) row at a time.  T1: the row is brought into the warp's shared-memory slot
 //       by one 1-D TMA bulk copy (cp.async.bulk, completion on an mbarrier); only the <= 15 head and
-//       tail bytes that are not 16-byte aligned in global memory are moved by the lanes.  T2: exact
-//       sum and sum of squares with IDP.4A over 16-byte groups.  T3: the cut collapses to two byte
-//       bounds, found by evaluating the exact 64/128-bit predicate for all 256 byte values across the
-//       warp.  T4: a packed range check (3 instructions per 32-bit word, VIADDMNMX.U16x2) finds the
-//       16-byte groups that contain a value outside [lo, hi]; their indices are compacted into a
-//       queue and only those groups are revisited byte by byte (replace, update S and Q
-//       incrementally).  T5: next threshold, on chip.  T6: one TMA bulk store.  HBM sees one read
-//       and one write per sample.
+//       tail bytes that are not 16-byte aligned in global memory are moved by the lanes.  T2: one
+//       pass over the row gives the exact sum and sum of squares (IDP.4A) and, per 16-byte group, its
+//       largest and smallest byte (VIMNMX3.U16x2) -- the group summaries.  T3: the cut collapses to
+//       two byte bounds, found by evaluating the exact 64/128-bit predicate on candidate byte values
+//       across the warp.  T4: a threshold sweep reads only the summaries (two bytes per group instead
+//       of sixteen): a packed test per sixteen groups, exact byte masks where it fires; a lane repairs
+//       the groups it found by itself (exact per-byte masks, replace, S and Q deltas, summary
+//       refresh), so there is no queue, atomic or barrier.  T5: next threshold, on chip, from the
+//       updated S, Q and summaries.  T6: one TMA bulk store.  HBM sees one read and one write per
+//       sample.
 //   td_u8_generic_kernel  any alignment / stride / row length / window, mean or median: one CTA per
 //       row, byte loads, iterations through global memory (L1/L2).  Correctness path, not tuned.
 #pragma once
@@ -34,46 +36,56 @@ struct TdU8Params {
   uint8_t* flags;             // optional [rows][S]
   unsigned long long* counts; // optional [n_thr]
   int slot_bytes;             // staged kernel: bytes per warp slot (multiple of 16)
-  int queue_entries;          // staged kernel: u16 entries per warp queue
+  int sum_entries;            // staged kernel: group summaries per team (a multiple of 16)
 };
 
 // ------------------------------------------------------------------------------------------------
 // staged hot path
 // ------------------------------------------------------------------------------------------------
 
-// Packed range check of one 16-byte group.  For a 32-bit word w, the u16 lanes of w and of w<<8
-// carry every byte once as the HIGH byte of a lane, so with LB = lo<<8 a byte lies outside [lo, hi]
-// <=> its lane satisfies ((v - LB) mod 2^16) > ((hi-lo)<<8 | 0xFF).  VIADDMNMX.U16x2 does the
-// subtract and the running max in one instruction: 3 instructions per word, two chains per group.
-__device__ __forceinline__ uint32_t group_range_acc(const uint4& w, uint32_t negLB2) {
-  uint32_t a = __viaddmax_u16x2(w.x, negLB2, 0u);
-  uint32_t b = __viaddmax_u16x2(w.z, negLB2, 0u);
-  a = __viaddmax_u16x2(w.x << 8, negLB2, a);
-  b = __viaddmax_u16x2(w.z << 8, negLB2, b);
-  a = __viaddmax_u16x2(w.y, negLB2, a);
-  b = __viaddmax_u16x2(w.w, negLB2, b);
-  a = __viaddmax_u16x2(w.y << 8, negLB2, a);
-  b = __viaddmax_u16x2(w.w << 8, negLB2, b);
-  return __vmaxu2(a, b);
+// Group summaries.  Pass T2 leaves, for every 16-byte group of the row, its largest and its smallest byte
+// (two byte arrays gmax[], gmin[]).  A cut with kept interval [lo, hi] touches a group iff max > hi or
+// min < lo, so the threshold sweeps read two bytes per group instead of sixteen.  For a 32-bit word w the u16 lanes of w and of w << 8 carry every
+// byte once as the HIGH byte of a lane (the low byte is junk that cannot change the order of the high
+// bytes), so VIMNMX3.U16x2 over {x, y, z, w, x<<8, y<<8, z<<8, w<<8} gives the lane with the largest / smallest byte.
+__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+  uint32_t d;
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));   // selector bit 3 = replicate sign
+  return d;
 }
-
-// Append a group index to the warp's hit queue.  Plain shared-memory atomic (inline PTX so that the
-// compiler does not wrap it in a ballot/REDUX aggregation): hits are rare, one or two lanes per step.
-__device__ __forceinline__ void queue_push(uint32_t tail_addr, uint16_t* queue, int gi) {
-  uint32_t at;
-  asm volatile("atom.shared.add.u32 %0, [%1], 1;" : "=r"(at) : "r"(tail_addr) : "memory");
-  queue[at] = (uint16_t)gi;
+__device__ __forceinline__ uint32_t group_summary(const uint4& w) {
+  const uint32_t x0 = w.x << 8, x1 = w.y << 8, x2 = w.z << 8, x3 = w.w << 8;
+  uint32_t mx = __vimax3_u16x2(w.x, w.y, w.z), mn = __vimin3_u16x2(w.x, w.y, w.z);
+  mx = __vimax3_u16x2(mx, w.w, x0); mn = __vimin3_u16x2(mn, w.w, x0);
+  mx = __vimax3_u16x2(mx, x1, x2);  mn = __vimin3_u16x2(mn, x1, x2);
+  mx = __vmaxu2(mx, x3);            mn = __vminu2(mn, x3);
+  mx = __vmaxu2(mx, prmt(mx, mx, 0x1032u));                   // both lanes: the lane with the largest high byte
+  mn = __vminu2(mn, prmt(mn, mn, 0x1032u));
+  return prmt(mx, mn, 0x4415u);                               // byte 1 = max byte, byte 0 = min byte
+}
+// the same for the four words of a group held by four neighbouring lanes (fix path): summary in every lane
+__device__ __forceinline__ uint32_t quad_summary(uint32_t w, uint32_t mask) {
+  const uint32_t x = w << 8;
+  uint32_t mx = __vmaxu2(w, x), mn = __vminu2(w, x);
+  mx = __vmaxu2(mx, __shfl_xor_sync(mask, mx, 1)); mn = __vminu2(mn, __shfl_xor_sync(mask, mn, 1));
+  mx = __vmaxu2(mx, __shfl_xor_sync(mask, mx, 2)); mn = __vminu2(mn, __shfl_xor_sync(mask, mn, 2));
+  mx = __vmaxu2(mx, prmt(mx, mx, 0x1032u));
+  mn = __vminu2(mn, prmt(mn, mn, 0x1032u));
+  return prmt(mx, mn, 0x4415u);
+}
+// byte masks (0xFF per byte) of the bytes of w that are > hi / < lo; cab2 = 0x7fff - hi, cbe2 = 0x7fff + lo in
+// both u16 halves: lane + cab2 has bit 15 set iff byte > hi, cbe2 - lane has bit 15 set iff byte < lo
+__device__ __forceinline__ uint32_t bytes_above(uint32_t w, uint32_t cab2) {
+  return prmt(prmt(w, 0u, 0x4240u) + cab2, prmt(w, 0u, 0x4341u) + cab2, 0xFBD9u);
+}
+__device__ __forceinline__ uint32_t bytes_below(uint32_t w, uint32_t cbe2) {
+  return prmt(cbe2 - prmt(w, 0u, 0x4240u), cbe2 - prmt(w, 0u, 0x4341u), 0xFBD9u);
 }
 
 // Exact mask (0xFF per byte) of the bytes of w outside [lo, hi], 9 instructions: the bytes are spread
 // over two words of u16 lanes; lane + (0x7FFF - hi) sets bit 15 iff byte > hi, lane + (0x8000 - lo)
 // sets bit 15 iff byte >= lo; PRMT's sign-replicate mode turns the four bit-15 flags into a byte mask.
 // chi2 / clo2 hold those constants in both halves.  With lo = 1, hi = 0 every byte is marked.
-__device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
-  uint32_t d;
-  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));   // selector bit 3 = replicate sign
-  return d;
-}
 __device__ __forceinline__ uint32_t bytes_outside(uint32_t w, uint32_t chi2, uint32_t clo2) {
   const uint32_t xe = prmt(w, 0u, 0x4240u), xo = prmt(w, 0u, 0x4341u);
   const uint32_t fe = (xe + chi2) | ~(xe + clo2);
@@ -140,7 +152,7 @@ __device__ __forceinline__ void team_sum3(uint32_t& a, uint32_t& b, uint32_t& c,
   xsel ^= 1;
 }
 
-// control block per team (bytes): [0] mbarrier, [8] queue tail, [16] exchange 2 x kTeam(<=2) x 4 u32
+// control block per team (bytes): [0] mbarrier, [16] exchange 2 x kTeam(<=2) x 4 u32
 constexpr int kCtrlBytes = 16 + 2 * 2 * 4 * 4;
 
 // geometry of one row inside its slot: row byte i lives at slot[h + i]
@@ -173,18 +185,18 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
   const int tl = threadIdx.x % TL;                                // thread index inside the team
   const int wt = tl >> 5;                                         // warp index inside the team
   const int nteams = blockDim.x / TL;
+  // shared memory: [slots][group summaries][control blocks], one of each per team
   uint8_t* slot = smem + (size_t)team * P.slot_bytes;
-  uint16_t* queue = reinterpret_cast<uint16_t*>(smem + (size_t)nteams * P.slot_bytes) + (size_t)team * P.queue_entries;
-  uint8_t* ctrl = smem + (size_t)nteams * P.slot_bytes + (size_t)nteams * P.queue_entries * sizeof(uint16_t) +
-                  (size_t)team * kCtrlBytes;
+  uint8_t* base = smem + (size_t)nteams * P.slot_bytes;
+  uint8_t* gmax = base + (size_t)team * P.sum_entries * 2;        // largest byte of every 16-byte group
+  uint8_t* gmin = gmax + P.sum_entries;                           // smallest byte
+  base += (size_t)nteams * P.sum_entries * 2;
+  uint8_t* ctrl = base + (size_t)team * kCtrlBytes;
   uint64_t* bar = reinterpret_cast<uint64_t*>(ctrl);
-  volatile uint32_t* qtail = reinterpret_cast<volatile uint32_t*>(ctrl + 8);
   volatile uint32_t* xchg = reinterpret_cast<volatile uint32_t*>(ctrl + 16);
-  const uint32_t qtail_addr = smem_addr(ctrl + 8);
   if (tl == 0) {
     mbar_init(bar, 1);
     fence_mbar_init();
-    *qtail = 0;
   }
   team_sync<kTeam>(team);
 
@@ -193,6 +205,8 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
   int xsel = 0;
   const uint4* s4 = reinterpret_cast<const uint4*>(slot);
   uint32_t* s32 = reinterpret_cast<uint32_t*>(slot);
+  const uint4* gmax4 = reinterpret_cast<const uint4*>(gmax);
+  const uint4* gmin4 = reinterpret_cast<const uint4*>(gmin);
   const int64_t total_teams = (int64_t)gridDim.x * nteams;
   for (int64_t row = (int64_t)blockIdx.x * nteams + team; row < P.rows; row += total_teams) {
     // ---------------------------------------------------------------- T1: load
@@ -213,13 +227,15 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
       if (geo.a1 + t < S) slot[h + geo.a1 + t] = g[geo.a1 + t];  // tail bytes
       if (t < geo.pe) slot[h + S + t] = g[S - 1];
     }
+    const int J16 = (J + 15) >> 4;                                // summaries are swept sixteen at a time
+    if (tl < 16 && J + tl < 16 * J16) { gmax[J + tl] = 0; gmin[J + tl] = 255; }   // neutral: no cut touches them
     if (geo.body > 0) {
       mbar_wait(bar, phase);
       phase ^= 1;
     }
     team_sync<kTeam>(team);
 
-    // ---------------------------------------------------------------- T2: statistics
+    // ---------------------------------------------------------------- T2: statistics and group summaries
     uint32_t s1 = 0, s2 = 0, s3 = 0;
     {
       uint32_t s1b = 0, s2b = 0;
@@ -230,6 +246,9 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
         s1b = __dp4a(w.y, 0x01010101u, s1b); s2b = __dp4a(w.y, w.y, s2b);
         s1 = __dp4a(w.z, 0x01010101u, s1); s2 = __dp4a(w.z, w.z, s2);
         s1b = __dp4a(w.w, 0x01010101u, s1b); s2b = __dp4a(w.w, w.w, s2b);
+        const uint32_t e = group_summary(w);
+        gmax[gi] = (uint8_t)(e >> 8);
+        gmin[gi] = (uint8_t)e;
       }
       s1 += s1b; s2 += s2b;
     }
@@ -238,96 +257,90 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
     uint32_t xf = slot[h], xl = slot[h + S - 1];
     uint64_t Ssum = s1 - (uint32_t)h * xf - (uint32_t)geo.pe * xl;
     uint64_t Qsum = (uint64_t)s2 - (uint64_t)((uint32_t)h * xf * xf) - (uint64_t)((uint32_t)geo.pe * xl * xl);
-    uint32_t qbase = 0;                                           // queue tail only grows within a row
 
     // ---------------------------------------------------------------- T3..T5: thresholds, on chip
+    uint4* s4w = reinterpret_cast<uint4*>(slot);
     for (int it = 0; it < P.n_thr; ++it) {
-      // T3: exact kept interval [lo, hi] and replacement value for this snapshot (every warp of the
-      // team computes the same scalars: cheaper than another barrier)
+      // T3: exact kept interval [lo, hi] for this snapshot (every warp of the team computes the same
+      // scalars: cheaper than another barrier)
       int lo, hi;
       const uint64_t V = (uint64_t)S * Qsum - Ssum * Ssum;
       const U8Cut cut = make_cut_u8((uint32_t)S, Ssum, V, P.p[it]);
       warp_bounds_u8_fast(cut, P.pf[it], V, lane, lo, hi);
       if (lo == 0 && hi == 255) continue;                        // nothing can be cut
-      const uint32_t r = rounded_mean_u8((uint32_t)S, Ssum);
-      const bool all = lo > hi;                                  // empty kept interval: everything is cut
-      int qn;
-      if (!all) {
-        // T4a: packed range check; queue the groups that hold a value outside [lo, hi]
-        const uint32_t neg = (0x10000u - ((uint32_t)lo << 8)) & 0xffffu;
-        const uint32_t negLB2 = neg | (neg << 16);
-        const uint32_t thr = ((uint32_t)(hi - lo) << 8) | 0xffu;
-        const uint32_t thr2 = thr | (thr << 16);
-        uint16_t* q = queue - qbase;                             // entries of this iteration start at queue[0]
-        // four groups per thread in flight (independent loads and compare chains)
-        int g0 = 0;
-        for (; g0 + 4 * TL <= J; g0 += 4 * TL) {
-          const int gi = g0 + tl;
-          const uint4 w0 = s4[gi], w1 = s4[gi + TL], w2 = s4[gi + 2 * TL], w3 = s4[gi + 3 * TL];
-          const bool h0 = __vmaxu2(group_range_acc(w0, negLB2), thr2) != thr2;
-          const bool h1 = __vmaxu2(group_range_acc(w1, negLB2), thr2) != thr2;
-          const bool h2 = __vmaxu2(group_range_acc(w2, negLB2), thr2) != thr2;
-          const bool h3 = __vmaxu2(group_range_acc(w3, negLB2), thr2) != thr2;
-          if (h0) queue_push(qtail_addr, q, gi);
-          if (h1) queue_push(qtail_addr, q, gi + TL);
-          if (h2) queue_push(qtail_addr, q, gi + 2 * TL);
-          if (h3) queue_push(qtail_addr, q, gi + 3 * TL);
-        }
-        for (; g0 < J; g0 += TL) {
-          const int gi = g0 + tl;
-          if (gi < J && __vmaxu2(group_range_acc(s4[gi], negLB2), thr2) != thr2) queue_push(qtail_addr, q, gi);
-        }
-        team_sync<kTeam>(team);
-        const uint32_t tail = *qtail;
-        qn = (int)(tail - qbase);
-        qbase = tail;
-      } else {
-        for (int gi = tl; gi < J; gi += TL) queue[gi] = (uint16_t)gi;
-        qn = J;
-        team_sync<kTeam>(team);
-      }
-      if (qn == 0) continue;
-      // T4b: revisit the queued groups, one 32-bit word per thread (8 groups per warp step)
-      const uint32_t r4 = r * 0x01010101u;
+      const bool upd = it + 1 < P.n_thr;                         // later sweeps need fresh summaries
+      const uint32_t HI2 = (((uint32_t)(hi & 0xff) << 8) | 0xffu) * 0x00010001u;
+      const uint32_t LO2 = ((uint32_t)lo << 8) * 0x00010001u;
+      const uint32_t cab2 = (0x7fffu - (uint32_t)(hi & 0xff)) * 0x00010001u;
+      const uint32_t cbe2 = (0x7fffu + (uint32_t)lo) * 0x00010001u;
       const uint32_t chi2 = (0x7fffu - (uint32_t)hi) * 0x00010001u;
       const uint32_t clo2 = (0x8000u - (uint32_t)lo) * 0x00010001u;
+      uint32_t r = 0, r4 = 0;
+      bool have_r = false;
       uint32_t cnt = 0, sx = 0, sxx = 0;
-      auto fix_word = [&](int widx, uint32_t w) {
+      // T4b: a lane repairs a whole 16-byte group by itself: exact byte masks, replace, accumulate the
+      // deltas of S and Q, refresh the group's summary.  Groups are private to the lane that swept their
+      // summaries, so no queue, atomic or barrier is involved.
+      auto fix_word = [&](uint32_t w, int widx) -> uint32_t {   // branch-free: most lanes see m == 0
         const uint32_t m = bytes_outside(w, chi2, clo2);
-        if (m) {
-          const uint32_t f = w & m;
-          cnt += __popc(m);                                       // 8 per byte; divided below
-          sx = __dp4a(f, 0x01010101u, sx);
-          sxx = __dp4a(f, f, sxx);
-          s32[widx] = (w & ~m) | (r4 & m);
-          if (kFlags) {
+        const uint32_t f = w & m;
+        cnt += __popc(m);                                         // 8 per byte; divided below
+        sx = __dp4a(f, 0x01010101u, sx);
+        sxx = __dp4a(f, f, sxx);
+        if (kFlags && m) {
 #pragma unroll
-            for (int j = 0; j < 4; ++j) {
-              const int i = widx * 4 + j - h;
-              if (((m >> (8 * j)) & 1u) && (unsigned)i < (unsigned)S) P.flags[row * S + i] = 1;
-            }
+          for (int j = 0; j < 4; ++j) {
+            const int i = widx * 4 + j - h;
+            if (((m >> (8 * j)) & 1u) && (unsigned)i < (unsigned)S) P.flags[row * S + i] = 1;
           }
         }
+        return (w & ~m) | (r4 & m);
       };
-      constexpr int EPS = 8 * kTeam;                              // entries per team step
-      int e0 = 0;
-      for (; e0 + 2 * EPS <= qn; e0 += 2 * EPS) {                 // two independent entries per thread
-        const int ea = e0 + (tl >> 2);
-        const int wa = (int)queue[ea] * 4 + (tl & 3), wb = (int)queue[ea + EPS] * 4 + (tl & 3);
-        const uint32_t va = s32[wa], vb = s32[wb];
-        fix_word(wa, va);
-        fix_word(wb, vb);
-      }
-      for (; e0 < qn; e0 += EPS) {
-        const int e = e0 + (tl >> 2);
-        if (e < qn) {
-          const int widx = (int)queue[e] * 4 + (tl & 3);
-          fix_word(widx, s32[widx]);
+      // T4a: sweep the group summaries, sixteen groups per lane and step
+      for (int ub = 0; ub < J16; ub += TL) {
+        const int u = ub + tl;
+        uint4 a = make_uint4(0u, 0u, 0u, 0u), b = make_uint4(~0u, ~0u, ~0u, ~0u);
+        if (u < J16) { a = gmax4[u]; b = gmin4[u]; }
+        uint32_t ah = __vimax3_u16x2(a.x, a.y, a.z), al = __vimin3_u16x2(b.x, b.y, b.z);
+        ah = __vimax3_u16x2(ah, a.w, a.x << 8);      al = __vimin3_u16x2(al, b.w, b.x << 8);
+        ah = __vimax3_u16x2(ah, a.y << 8, a.z << 8); al = __vimin3_u16x2(al, b.y << 8, b.z << 8);
+        ah = __vimax3_u16x2(ah, a.w << 8, HI2);      al = __vimin3_u16x2(al, b.w << 8, LO2);
+        const bool hit = ah != HI2 || al != LO2;
+        if (!__any_sync(FULL, hit)) continue;
+        if (!have_r) {
+          r = rounded_mean_u8((uint32_t)S, Ssum);
+          r4 = r * 0x01010101u;
+          have_r = true;
+        }
+        if (hit) {
+          // exact hit mask: bit j <=> group 16 u + j holds a value outside [lo, hi]
+          const uint32_t m0 = bytes_above(a.x, cab2) | bytes_below(b.x, cbe2);
+          const uint32_t m1 = bytes_above(a.y, cab2) | bytes_below(b.y, cbe2);
+          const uint32_t m2 = bytes_above(a.z, cab2) | bytes_below(b.z, cbe2);
+          const uint32_t m3 = bytes_above(a.w, cab2) | bytes_below(b.w, cbe2);
+          uint32_t hm = (((m0 & 0x01010101u) * 0x01020408u) >> 24) | ((((m1 & 0x01010101u) * 0x01020408u) >> 24) << 4) |
+                        ((((m2 & 0x01010101u) * 0x01020408u) >> 24) << 8) | ((((m3 & 0x01010101u) * 0x01020408u) >> 24) << 12);
+          while (hm) {
+            const int gi = u * 16 + __ffs(hm) - 1;
+            hm &= hm - 1;
+            uint4 w = s4w[gi];
+            w.x = fix_word(w.x, gi * 4 + 0);
+            w.y = fix_word(w.y, gi * 4 + 1);
+            w.z = fix_word(w.z, gi * 4 + 2);
+            w.w = fix_word(w.w, gi * 4 + 3);
+            s4w[gi] = w;
+            if (upd) {
+              const uint32_t e = group_summary(w);
+              gmax[gi] = (uint8_t)(e >> 8);
+              gmin[gi] = (uint8_t)e;
+            }
+          }
         }
       }
       team_sum3<kTeam>(cnt, sx, sxx, xchg, xsel, wt, lane, team);  // also orders the fixes before the next sweep
       cnt >>= 3;
       if (cnt) {
+        if (!have_r) r = rounded_mean_u8((uint32_t)S, Ssum);     // the hits were in another warp of the team
         // take the padding copies out again: they were cut iff their original was
         const bool ff = (int)xf < lo || (int)xf > hi, fl = (int)xl < lo || (int)xl > hi;
         if (ff) { cnt -= h; sx -= h * xf; sxx -= h * xf * xf; xf = r; }
@@ -352,10 +365,7 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
       const int t = tl - 16;
       if (geo.a1 + t < S) go[geo.a1 + t] = slot[h + geo.a1 + t];
     }
-    if (tl == 0) {
-      if (geo.body > 0) bulk_wait_read<0>();                      // slot may be overwritten after this
-      *qtail = 0;
-    }
+    if (tl == 0 && geo.body > 0) bulk_wait_read<0>();             // slot may be overwritten after this
     team_sync<kTeam>(team);
   }
 }
