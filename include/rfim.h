@@ -73,7 +73,8 @@ typedef struct {
   int32_t   variant;       /* 0 = auto.  Non-zero selects a kernel variant (testing / tuning):
                               1 = generic (any alignment, any row length), 2 = fast path (staged TDSC /
                               cluster FDSC), 3 / 4 = staged TDSC with one / two warps per row,
-                              5 / 6 / 7 / 8 = cluster FDSC with 1 / 2 / 4 / 8 CTAs per tile.
+                              5 / 6 / 7 / 8 = cluster FDSC with 1 / 2 / 4 / 8 CTAs per tile, 11 / 12 = the same with
+                              4 / 8 CTAs and one thread per word column.
                               A variant that cannot run the request returns RFIM_ERR_UNSUPPORTED.  */
   int32_t   reserved;      /* must be 0                                                            */
 } rfim_opts;               /* opts == NULL means all zeros                                          */

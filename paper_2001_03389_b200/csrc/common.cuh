@@ -91,6 +91,30 @@ __device__ __forceinline__ void thread_bounds_u8(const U8Cut& c, int& lo, int& h
   hi = a;
 }
 
+// Same interval for ONE thread in closed form: with T = isqrt(W) (floor), |N x - S| <= T <=> (N x - S)^2 <= W,
+// so the kept values are ceil((S - T) / N) <= x <= floor((S + T) / N), clamped to 0..255.  The square root is
+// taken in fp64 and corrected with exact integer checks; the quotients are float estimates corrected the same
+// way.  Result identical to warp_bounds_u8 (empty interval: lo = 1, hi = 0).
+__device__ __forceinline__ uint32_t div_floor_u64(uint64_t a, uint32_t n) {   // a / n, quotient < 2^24 * 512
+  uint64_t q = (uint64_t)__fdividef((float)a, (float)n);
+  while (q * n > a) --q;
+  while (a - q * n >= n) ++q;
+  return (uint32_t)q;
+}
+__device__ __forceinline__ void thread_bounds_u8_sqrt(const U8Cut& c, int& lo, int& hi) {
+  if (c.never) { lo = 0; hi = 255; return; }
+  uint64_t T = (uint64_t)__dsqrt_rd((double)c.W);              // within 1 of floor(sqrt(W)), below 2^32
+  if (T > 0xffffffffull) T = 0xffffffffull;
+  while (T * T > c.W) --T;
+  while (T < 0xffffffffull && (T + 1) * (T + 1) <= c.W) ++T;
+  const uint64_t S = c.S, N = c.N;
+  const uint64_t top = S + T;                                  // < 2^33
+  const uint64_t hq = top >= 256ull * N ? 255ull : div_floor_u64(top, c.N);
+  hi = (int)(hq > 255ull ? 255ull : hq);
+  lo = S > T ? (int)div_floor_u64(S - T + N - 1, c.N) : 0;     // ceil((S - T) / N), <= 255 because S <= 255 N
+  if (lo > hi) { lo = 1; hi = 0; }
+}
+
 __device__ __forceinline__ uint32_t warp_sum_u32(uint32_t v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);

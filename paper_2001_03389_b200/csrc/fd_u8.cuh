@@ -90,7 +90,7 @@ __device__ __forceinline__ uint32_t dsmem_addr(const void* local, uint32_t rank)
 }
 __device__ __forceinline__ uint32_t dsmem_ld_u32(uint32_t addr) {
   uint32_t v;
-  asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(addr) : "memory");
+  asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(addr));
   return v;
 }
 __device__ __forceinline__ uint4 dsmem_ld_u128(uint32_t addr) {
@@ -100,6 +100,23 @@ __device__ __forceinline__ uint4 dsmem_ld_u128(uint32_t addr) {
                : "r"(addr)
                : "memory");
   return v;
+}
+
+// colS += sum over the cluster of *pS, colQ += sum of *pQ.  All (up to 16) remote loads are issued before the
+// first is consumed: a DSMEM load takes about 200 cycles, a loop of dependent adds would pay that per CTA.
+__device__ __forceinline__ void cluster_gather2(const uint32_t* pS, const uint32_t* pQ, uint32_t ncta, uint32_t& colS,
+                                                uint32_t& colQ) {
+  uint32_t vs[8], vq[8];
+#pragma unroll
+  for (uint32_t q = 0; q < 8; ++q) {
+    vs[q] = 0; vq[q] = 0;
+    if (q < ncta) {
+      vs[q] = dsmem_ld_u32(dsmem_addr(pS, q));
+      vq[q] = dsmem_ld_u32(dsmem_addr(pQ, q));
+    }
+  }
+#pragma unroll
+  for (uint32_t q = 0; q < 8; ++q) { colS += vs[q]; colQ += vq[q]; }
 }
 
 // Kept interval for one cut, ONE thread: float estimate of mu -/+ k sigma, then a short walk on the
@@ -151,8 +168,12 @@ __host__ __device__ inline size_t fd_cluster_smem_bytes(int PW, int Rq, int WC) 
   return (size_t)Rq * PW * 4 + fd_cluster_ctrl_bytes(WC);
 }
 
-template <int PW>
-__global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params P) {
+// RG = row groups that share a warp: RG = 4 maps a warp to 8 word columns x 4 row groups (512 threads for a
+// 128-word tile, each thread sees every 4th row of the CTA); RG = 1 maps a thread to one word column and
+// ALL rows of the CTA (128 threads): four times the work per thread, so the per-tile overhead (bounds,
+// exchanges, barriers, copies) is amortised over four times as many words, and no shuffles are needed.
+template <int PW, int RG>
+__global__ void __launch_bounds__(128 * RG, 2) fd_u8_cluster_kernel(const FdU8Params P) {
   extern __shared__ __align__(128) uint8_t smem[];
   const int C = P.C, Ts = P.Ts, WC = P.WC, Rq = P.Rq, TsP = 4 * WC;
   uint32_t* tile = reinterpret_cast<uint32_t*>(smem);
@@ -167,12 +188,11 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
   volatile uint32_t* any_empty = reinterpret_cast<volatile uint32_t*>(bar + 1);
 
   const int tid = threadIdx.x, nthreads = blockDim.x, lane = tid & 31;
-  const int j = (tid >> 5) * 8 + (lane & 7);          // word column of this thread
-  const int rg = lane >> 3;                           // row group 0..3
+  const int j = RG == 4 ? (tid >> 5) * 8 + (lane & 7) : tid;   // word column of this thread
+  const int rg0 = RG == 4 ? lane >> 3 : 0;            // first row group of this thread (it owns rg0, rg0 + RG, .. < 4)
   const uint32_t rank = cluster_ctarank(), ncta = cluster_nctarank();
   const int c0 = (int)rank * Rq;                      // first channel of this CTA
   const int nrows = max(0, min(Rq, C - c0));
-  const int ni = nrows > rg ? (nrows - rg + kFdRG - 1) / kFdRG : 0;   // rows rg + 4 i of this thread
   const int wpc = (WC + (int)ncta - 1) / (int)ncta;   // word columns owned per CTA (F3)
   const int nload = min(nrows, nthreads);
 
@@ -211,14 +231,19 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
     mbar_wait(bar, phase);
     phase ^= 1;
 
-    // word offset of column s0 inside the shared-memory rows of this thread (same for all its rows)
-    const int offw = (int)((reinterpret_cast<uintptr_t>(gsrc + (int64_t)rg * P.stride) & 15) >> 2);
-    uint32_t* const col0 = tile + (size_t)rg * PW + offw + j;
+    // rows rg + 4 i of one row group share the word offset of column s0 inside their shared-memory rows
+    auto group_rows = [&](int rg) { return nrows > rg ? (nrows - rg + kFdRG - 1) / kFdRG : 0; };
+    auto group_col0 = [&](int rg) {
+      const int offw = (int)((reinterpret_cast<uintptr_t>(gsrc + (int64_t)rg * P.stride) & 15) >> 2);
+      return tile + (size_t)rg * PW + offw + j;
+    };
 
     // ------------------------------------------------------------------ F2: column statistics
     {
       uint32_t S4[4] = {0, 0, 0, 0}, Q4[4] = {0, 0, 0, 0};
-      const uint32_t* col = col0;
+      for (int rg = rg0; rg < kFdRG; rg += RG) {
+      const int ni = group_rows(rg);
+      const uint32_t* col = group_col0(rg);
       int i = 0;
 #pragma unroll 2
       for (; i + 4 <= ni; i += 4, col += 16 * PW) {
@@ -240,12 +265,15 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
           S4[u] += x; Q4[u] += x * x;
         }
       }
-#pragma unroll
-      for (int u = 0; u < 4; ++u) {                    // reduce over the four row groups of the warp
-        S4[u] += __shfl_xor_sync(FULL, S4[u], 8);  Q4[u] += __shfl_xor_sync(FULL, Q4[u], 8);
-        S4[u] += __shfl_xor_sync(FULL, S4[u], 16); Q4[u] += __shfl_xor_sync(FULL, Q4[u], 16);
       }
-      if (rg == 0) {
+      if (RG == 4) {
+#pragma unroll
+        for (int u = 0; u < 4; ++u) {                  // reduce over the four row groups of the warp
+          S4[u] += __shfl_xor_sync(FULL, S4[u], 8);  Q4[u] += __shfl_xor_sync(FULL, Q4[u], 8);
+          S4[u] += __shfl_xor_sync(FULL, S4[u], 16); Q4[u] += __shfl_xor_sync(FULL, Q4[u], 16);
+        }
+      }
+      if (rg0 == 0) {
         reinterpret_cast<uint4*>(xS)[j] = make_uint4(S4[0], S4[1], S4[2], S4[3]);
         reinterpret_cast<uint4*>(xQ)[j] = make_uint4(Q4[0], Q4[1], Q4[2], Q4[3]);
       }
@@ -259,10 +287,7 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
     uint32_t colS = 0, colQ = 0;
     if (owner) {
       if (ncta > 1) {
-        for (uint32_t q = 0; q < ncta; ++q) {
-          colS += dsmem_ld_u32(dsmem_addr(&xS[ocol], q));
-          colQ += dsmem_ld_u32(dsmem_addr(&xQ[ocol], q));
-        }
+        cluster_gather2(&xS[ocol], &xQ[ocol], ncta, colS, colQ);
       } else {
         colS = xS[ocol];
         colQ = xQ[ocol];
@@ -277,7 +302,7 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
         if (ocol < tw) {
           const uint64_t V = (uint64_t)C * colQ - (uint64_t)colS * colS;
           const U8Cut cut = make_cut_u8((uint32_t)C, colS, V, P.p[it]);
-          thread_bounds_u8_fast(cut, P.pf[it], V, lo, hi);
+          thread_bounds_u8_sqrt(cut, lo, hi);
           r = rounded_mean_u8((uint32_t)C, colS);
         }
         lo_b[ocol] = (uint8_t)lo;
@@ -313,7 +338,7 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
       const bool need_stats = it + 1 < P.n_thr;
 
       uint32_t cnt4 = 0, sxE = 0, sxO = 0, sq[4] = {0, 0, 0, 0};   // per-column deltas of this thread, packed
-      auto fix_word = [&](uint32_t* ptr, uint32_t w, int i) {
+      auto fix_word = [&](uint32_t* ptr, uint32_t w, int rg, int i) {
         const uint32_t m = bytes_outside_cols(w, chiE, cloE, chiO, cloO);
         if (m == 0) return;
         *ptr = (w & ~m) | (r4 & m);
@@ -332,25 +357,45 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
             if ((m >> (8 * u)) & 1u) fl[u] = 1;
         }
       };
-      {
-        uint32_t* col = col0;
+      // Sweep first, repair afterwards: the packed test only records which four-row steps hold an outlier
+      // (one bit per step); the exact repair then runs over the set bits.  A warp step covers 512 bytes,
+      // so at k = 3 nearly every step has SOME lane with an outlier: repairing inside the sweep would make
+      // every lane pay the repair code at every step, while the deferred loop runs max-over-lanes(popcount)
+      // times (two or three for noise).
+      for (int rg = rg0; rg < kFdRG; rg += RG) {
+        const int ni = group_rows(rg);
+        uint32_t* const colb = group_col0(rg);
+        uint32_t* col = colb;
+        unsigned long long hm = 0ull;
         int i = 0;
-#pragma unroll 2
+#pragma unroll 4
         for (; i + 4 <= ni; i += 4, col += 16 * PW) {
           const uint32_t w0 = col[0], w1 = col[4 * PW], w2 = col[8 * PW], w3 = col[12 * PW];
           uint32_t aO = __viaddmax_u16x2(w0, negO, 0u), aE = __viaddmax_u16x2(w0 << 8, negE, 0u);
           uint32_t bO = __viaddmax_u16x2(w1, negO, 0u), bE = __viaddmax_u16x2(w1 << 8, negE, 0u);
           aO = __viaddmax_u16x2(w2, negO, aO); aE = __viaddmax_u16x2(w2 << 8, negE, aE);
           bO = __viaddmax_u16x2(w3, negO, bO); bE = __viaddmax_u16x2(w3 << 8, negE, bE);
-          aO = __vmaxu2(aO, bO); aE = __vmaxu2(aE, bE);
-          if (slow || __vmaxu2(aO, thrO) != thrO || __vmaxu2(aE, thrE) != thrE) {
-            fix_word(col, w0, i);
-            fix_word(col + 4 * PW, w1, i + 1);
-            fix_word(col + 8 * PW, w2, i + 2);
-            fix_word(col + 12 * PW, w3, i + 3);
-          }
+          aO = __vimax3_u16x2(aO, bO, thrO); aE = __vimax3_u16x2(aE, bE, thrE);
+          if (aO != thrO || aE != thrE) hm |= 1ull << (i >> 2);
         }
-        for (; i < ni; ++i, col += 4 * PW) fix_word(col, col[0], i);
+        if (slow) hm = ~0ull;
+        for (; i < ni; ++i, col += 4 * PW) fix_word(col, col[0], rg, i);
+        const int nsteps = ni >> 2;
+        if (nsteps < 64) hm &= (1ull << nsteps) - 1ull;
+        while (hm) {
+          const int st = __ffsll((long long)hm) - 1;
+          hm &= hm - 1ull;
+          uint32_t* c4 = colb + (size_t)st * 16 * PW;
+          const uint32_t w0 = c4[0], w1 = c4[4 * PW], w2 = c4[8 * PW], w3 = c4[12 * PW];
+          // usually one of the four rows holds the outlier (a narrow-band RFI channel): packed test per word
+          auto hit = [&](uint32_t w) {
+            return slow || __viaddmax_u16x2(w, negO, thrO) != thrO || __viaddmax_u16x2(w << 8, negE, thrE) != thrE;
+          };
+          if (hit(w0)) fix_word(c4, w0, rg, 4 * st);
+          if (hit(w1)) fix_word(c4 + 4 * PW, w1, rg, 4 * st + 1);
+          if (hit(w2)) fix_word(c4 + 8 * PW, w2, rg, 4 * st + 2);
+          if (hit(w3)) fix_word(c4 + 12 * PW, w3, rg, 4 * st + 3);
+        }
       }
 
       if (need_stats || P.counts) {
@@ -363,12 +408,14 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
           dQ[u] = c * r * r - sq[u];
           cnt += c;
         }
+        if (RG == 4) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u) {
-          dS[u] += __shfl_xor_sync(FULL, dS[u], 8);  dQ[u] += __shfl_xor_sync(FULL, dQ[u], 8);
-          dS[u] += __shfl_xor_sync(FULL, dS[u], 16); dQ[u] += __shfl_xor_sync(FULL, dQ[u], 16);
+          for (int u = 0; u < 4; ++u) {
+            dS[u] += __shfl_xor_sync(FULL, dS[u], 8);  dQ[u] += __shfl_xor_sync(FULL, dQ[u], 8);
+            dS[u] += __shfl_xor_sync(FULL, dS[u], 16); dQ[u] += __shfl_xor_sync(FULL, dQ[u], 16);
+          }
         }
-        if (need_stats && rg == 0) {
+        if (need_stats && rg0 == 0) {
           reinterpret_cast<uint4*>(xS)[j] = make_uint4(dS[0], dS[1], dS[2], dS[3]);
           reinterpret_cast<uint4*>(xQ)[j] = make_uint4(dQ[0], dQ[1], dQ[2], dQ[3]);
         }
@@ -381,10 +428,7 @@ __global__ void __launch_bounds__(512, 2) fd_u8_cluster_kernel(const FdU8Params 
         if (ncta > 1) cluster_sync_all(); else __syncthreads();
         if (owner) {
           if (ncta > 1) {
-            for (uint32_t q = 0; q < ncta; ++q) {
-              colS += dsmem_ld_u32(dsmem_addr(&xS[ocol], q));
-              colQ += dsmem_ld_u32(dsmem_addr(&xQ[ocol], q));
-            }
+            cluster_gather2(&xS[ocol], &xQ[ocol], ncta, colS, colQ);
           } else {
             colS += xS[ocol];
             colQ += xQ[ocol];

@@ -70,7 +70,7 @@ int validate(int op, void* data, int beams, int channels, int samples, rfim_dtyp
   if (z.reserved != 0) return RFIM_ERR_INVALID;
   if (z.sample_stride != 0 && z.sample_stride < samples) return RFIM_ERR_INVALID;
   if (z.window < 0 || z.bin_size < 0) return RFIM_ERR_INVALID;
-  if (z.variant < 0 || z.variant > 8) return RFIM_ERR_INVALID;
+  if (z.variant < 0 || z.variant > 12) return RFIM_ERR_INVALID;
   if (op == 1 && z.bin_size != 0) {
     if (z.bin_size > channels || channels % z.bin_size != 0) return RFIM_ERR_INVALID;
     if (dtype == RFIM_U8 && z.bin_size != channels && z.bin_size > 65536) return RFIM_ERR_INVALID;
@@ -250,61 +250,62 @@ int launch_td_f32(const Call& c) {
 
 // ------------------------------------------------------------------------------------------ FD u8
 // Geometry of the cluster kernel for the request, or false when only the generic kernel can run it.
-struct FdPlan { int cl, pw, ts, wc, rq, tiles_per_beam, smem; };
+struct FdPlan { int cl, pw, ts, wc, rq, rg, tiles_per_beam, smem; };
 
 constexpr int kFdPw[] = {136, 120, 104, 88, 72, 56, 40, 24};    // row pitches (words), PW mod 32 in {8, 24}
 
-bool plan_fd_u8_for(const Call& c, int cl, size_t budget, FdPlan& pl) {
+bool plan_fd_u8_for(const Call& c, int cl, int rg, size_t budget, FdPlan& pl) {
   const int rq = (c.channels + cl - 1) / cl;
-  if (rq > 1020) return false;                                   // packed per-thread delta counters (255 rows/thread)
+  if (rq > 255 * rg) return false;                               // packed per-thread delta counters (255 rows/thread)
+  if (rg == 1 && cl < 4) return false;                           // column owners: 4 * ceil(WC / cl) threads <= WC
   for (int pw : kFdPw) {
     int ts_max = 4 * pw - 16;
     if (ts_max > 512) ts_max = 512;                              // 4 * WC <= 512 threads
     const int tiles = (c.samples + ts_max - 1) / ts_max;
     int ts = (c.samples + tiles - 1) / tiles;
     ts = (ts + 3) & ~3;
-    const int wc = ((ts / 4) + 7) & ~7;
+    const int wc = rg == 1 ? ((ts / 4) + 31) & ~31 : ((ts / 4) + 7) & ~7;   // blockDim = rg * wc, whole warps
     const size_t smem = rfim::fd_cluster_smem_bytes(pw, rq, wc);
     if (smem > budget) continue;
-    pl.cl = cl; pl.pw = pw; pl.ts = ts; pl.wc = wc; pl.rq = rq; pl.tiles_per_beam = tiles; pl.smem = (int)smem;
+    pl.cl = cl; pl.pw = pw; pl.ts = ts; pl.wc = wc; pl.rq = rq; pl.rg = rg; pl.tiles_per_beam = tiles; pl.smem = (int)smem;
     return true;
   }
   return false;
 }
 
-bool plan_fd_u8_cluster(const Call& c, int force_cl, FdPlan& pl) {
+bool plan_fd_u8_cluster(const Call& c, int force_cl, int rg, FdPlan& pl) {
   if (c.policy != RFIM_REPLACE_MEAN || c.bin_size != c.channels) return false;
   const uintptr_t src = reinterpret_cast<uintptr_t>(c.data), dst = reinterpret_cast<uintptr_t>(c.out);
   if ((src & 3) != 0 || (c.stride & 3) != 0) return false;       // 32-bit word columns
   if (((src ^ dst) & 15) != 0) return false;                     // aligned interiors of src and dst rows coincide
   if (c.channels > 60000) return false;                          // 32-bit column totals inside the kernel
   const size_t half = (size_t)(kMaxSmem + 1024) / 2 - 1024;      // two CTAs per SM (1 KB reserved per CTA)
-  if (force_cl) return plan_fd_u8_for(c, force_cl, half, pl) || plan_fd_u8_for(c, force_cl, (size_t)kMaxSmem, pl);
+  if (force_cl) return plan_fd_u8_for(c, force_cl, rg, half, pl) || plan_fd_u8_for(c, force_cl, rg, (size_t)kMaxSmem, pl);
   // smallest cluster that still gets the widest tile with two CTAs per SM; else the widest tile any cluster gets
   FdPlan best; bool have = false;
   for (int cl = 1; cl <= 8; cl *= 2) {
     FdPlan p;
-    if (!plan_fd_u8_for(c, cl, half, p)) continue;
+    if (!plan_fd_u8_for(c, cl, rg, half, p)) continue;
     if (!have || p.ts > best.ts) { best = p; have = true; }
     if (p.pw == kFdPw[0]) break;
   }
   if (!have) {
-    for (int cl = 8; cl >= 1 && !have; cl /= 2) have = plan_fd_u8_for(c, cl, (size_t)kMaxSmem, best);
+    for (int cl = 8; cl >= 1 && !have; cl /= 2) have = plan_fd_u8_for(c, cl, rg, (size_t)kMaxSmem, best);
   }
   if (have) pl = best;
   return have;
 }
 
-template <int PW>
-int launch_fd_cluster(const Call& c, const FdPlan& pl, const rfim::FdU8Params& P, int sms) {
-  auto kernel = rfim::fd_u8_cluster_kernel<PW>;
+template <int PW, int RG>
+int launch_fd_cluster_rg(const Call& c, const FdPlan& pl, const rfim::FdU8Params& P, int sms) {
+  auto kernel = rfim::fd_u8_cluster_kernel<PW, RG>;
   CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem));
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = (unsigned)pl.cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-  cfg.blockDim = dim3((unsigned)(4 * pl.wc), 1, 1);
+  cfg.blockDim = dim3((unsigned)(RG * pl.wc), 1, 1);
   cfg.dynamicSmemBytes = (size_t)pl.smem;
   cfg.stream = c.stream;
   cfg.attrs = attr;
@@ -319,8 +320,13 @@ int launch_fd_cluster(const Call& c, const FdPlan& pl, const rfim::FdU8Params& P
   int st = clear_outputs(c);
   if (st != RFIM_OK) return st;
   CUDA_TRY(cudaLaunchKernelEx(&cfg, kernel, P));
-  static const char* names[4] = {"fd_u8_cluster1", "fd_u8_cluster2", "fd_u8_cluster4", "fd_u8_cluster8"};
-  return after_launch(names[pl.cl == 1 ? 0 : pl.cl == 2 ? 1 : pl.cl == 4 ? 2 : 3]);
+  static const char* names[2][4] = {{"fd_u8_cluster1", "fd_u8_cluster2", "fd_u8_cluster4", "fd_u8_cluster8"},
+                                    {"fd_u8_cluster1_rg1", "fd_u8_cluster2_rg1", "fd_u8_cluster4_rg1", "fd_u8_cluster8_rg1"}};
+  return after_launch(names[RG == 1][pl.cl == 1 ? 0 : pl.cl == 2 ? 1 : pl.cl == 4 ? 2 : 3]);
+}
+template <int PW>
+int launch_fd_cluster(const Call& c, const FdPlan& pl, const rfim::FdU8Params& P, int sms) {
+  return pl.rg == 1 ? launch_fd_cluster_rg<PW, 1>(c, pl, P, sms) : launch_fd_cluster_rg<PW, 4>(c, pl, P, sms);
 }
 
 int launch_fd_u8(const Call& c) {
@@ -339,9 +345,10 @@ int launch_fd_u8(const Call& c) {
   if (st != RFIM_OK) return st;
 
   FdPlan pl;
-  int force_cl = 0;
+  int force_cl = 0, rg = 4;
   if (c.variant >= 5 && c.variant <= 8) force_cl = 1 << (c.variant - 5);
-  const bool can_cluster = c.variant != 1 && plan_fd_u8_cluster(c, force_cl, pl);
+  if (c.variant >= 9 && c.variant <= 12) { force_cl = 1 << (c.variant - 9); rg = 1; }
+  const bool can_cluster = c.variant != 1 && plan_fd_u8_cluster(c, force_cl, rg, pl);
   if (c.variant >= 2 && !can_cluster) return RFIM_ERR_UNSUPPORTED;
   if (can_cluster) {
     P.Ts = pl.ts; P.WC = pl.wc; P.Rq = pl.rq;
