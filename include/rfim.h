@@ -72,9 +72,10 @@ typedef struct {
   void*     workspace;     /* device scratch of >= rfim_workspace_bytes(...) bytes, or NULL        */
   int32_t   variant;       /* 0 = auto.  Non-zero selects a kernel variant (testing / tuning):
                               1 = generic (any alignment, any row length), 2 = fast path (staged TDSC /
-                              cluster FDSC), 3 / 4 = staged TDSC with one / two warps per row,
-                              5 / 6 / 7 / 8 = cluster FDSC with 1 / 2 / 4 / 8 CTAs per tile, 11 / 12 = the same with
-                              4 / 8 CTAs and one thread per word column.
+                              strip FDSC), 3 / 4 = staged TDSC with one / two warps per row,
+                              5 / 6 / 7 / 8 = wide-tile cluster FDSC with 1 / 2 / 4 / 8 CTAs per tile, 11 / 12 =
+                              the same with 4 / 8 CTAs and one thread per word column, 13 = strip FDSC with
+                              per-row bulk copies, 14 = strip FDSC, never the whole tile in one CTA.
                               A variant that cannot run the request returns RFIM_ERR_UNSUPPORTED.  */
   int32_t   reserved;      /* must be 0                                                            */
 } rfim_opts;               /* opts == NULL means all zeros                                          */

@@ -9,6 +9,7 @@
 
 #include "common.cuh"
 #include "fd_u8.cuh"
+#include "fd_u8_strip.cuh"
 #include "td_f32.cuh"
 #include "td_u8.cuh"
 
@@ -70,7 +71,7 @@ int validate(int op, void* data, int beams, int channels, int samples, rfim_dtyp
   if (z.reserved != 0) return RFIM_ERR_INVALID;
   if (z.sample_stride != 0 && z.sample_stride < samples) return RFIM_ERR_INVALID;
   if (z.window < 0 || z.bin_size < 0) return RFIM_ERR_INVALID;
-  if (z.variant < 0 || z.variant > 12) return RFIM_ERR_INVALID;
+  if (z.variant < 0 || z.variant > 14) return RFIM_ERR_INVALID;
   if (op == 1 && z.bin_size != 0) {
     if (z.bin_size > channels || channels % z.bin_size != 0) return RFIM_ERR_INVALID;
     if (dtype == RFIM_U8 && z.bin_size != channels && z.bin_size > 65536) return RFIM_ERR_INVALID;
@@ -329,6 +330,131 @@ int launch_fd_cluster(const Call& c, const FdPlan& pl, const rfim::FdU8Params& P
   return pl.rg == 1 ? launch_fd_cluster_rg<PW, 1>(c, pl, P, sms) : launch_fd_cluster_rg<PW, 4>(c, pl, P, sms);
 }
 
+// strip kernel: all channels x 128 samples per tile, channels split over the smallest cluster whose CTAs fit
+// two to an SM (else one to an SM)
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*,
+                                  const cuuint64_t*, const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave,
+                                  CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+EncodeTiledFn encode_tiled_fn() {
+  static EncodeTiledFn fn = [] {
+    void* p = nullptr;
+    cudaDriverEntryPointQueryResult q;
+    if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) != cudaSuccess ||
+        q != cudaDriverEntryPointSuccess)
+      p = nullptr;
+    return reinterpret_cast<EncodeTiledFn>(p);
+  }();
+  return fn;
+}
+
+// one 2-D tensor per 16-byte alignment class k: rows k, k+4, ... of the [beams*channels][pitch] matrix, origin
+// rounded down to 16 bytes (off[k] bytes before the row start), box = 128 bytes x (channels per CTA) / 4 rows
+bool encode_strip_maps(const Call& c, uint8_t* base, int box_rows, CUtensorMap* maps, int* off) {
+  EncodeTiledFn enc = encode_tiled_fn();
+  if (!enc) return false;
+  for (int k = 0; k < 4; ++k) {
+    const uintptr_t addr = reinterpret_cast<uintptr_t>(base) + (uintptr_t)k * (uintptr_t)c.stride;
+    off[k] = (int)(addr & 15);
+    cuuint64_t dims[2] = {(cuuint64_t)c.samples + (cuuint64_t)off[k], (cuuint64_t)c.beams * (cuuint64_t)c.channels / 4};
+    cuuint64_t strides[1] = {(cuuint64_t)4 * (cuuint64_t)c.stride};
+    cuuint32_t box[2] = {(cuuint32_t)(rfim::kStripPitchW * 4), (cuuint32_t)box_rows};
+    cuuint32_t estr[2] = {1, 1};
+    if (enc(&maps[k], CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, reinterpret_cast<void*>(addr - off[k]), dims, strides, box,
+            estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+      return false;
+  }
+  return true;
+}
+
+struct StripPlan { int cl, rq, smem, box_rows, nw; bool tensor; };
+// rows per tensor copy: divides the Rq / 4 rows of a class, at most 256, and every box lands 128-byte aligned
+int strip_box_rows(int rq) {
+  const int rc = rq / 4;
+  for (int n = 1; n <= 8; ++n)
+    if (rc % n == 0 && rc / n <= 256 && ((rc / n) * rfim::kStripPitchW * 4) % 128 == 0) return rc / n;
+  return 0;
+}
+bool plan_fd_u8_strip(const Call& c, bool want_tensor, int force_cl, StripPlan& pl) {
+  if (c.policy != RFIM_REPLACE_MEAN || c.bin_size != c.channels) return false;
+  const uintptr_t src = reinterpret_cast<uintptr_t>(c.data), dst = reinterpret_cast<uintptr_t>(c.out);
+  if ((src & 3) != 0 || (c.stride & 3) != 0) return false;       // 32-bit word columns
+  if (((src ^ dst) & 15) != 0) return false;                     // aligned interiors of src and dst rows coincide
+  if (c.channels > 60000) return false;                          // 32-bit column totals inside the kernel
+  const size_t half = (size_t)(kMaxSmem + 1024) / 2 - 1024;      // two CTAs per SM (1 KB reserved per CTA)
+  // Order of preference (measured on config 4, in place): the whole tile in ONE CTA (one CTA per SM, 32 warps,
+  // no cluster barrier: 6.7 ms) before the smallest cluster whose CTAs fit two to an SM (7.1 ms with two CTAs),
+  // before the smallest cluster that fits at all.  force_cl: 0 = that order, -1 = skip the single-CTA choice.
+  for (int pass = 0; pass < 3; ++pass) {
+    for (int cl = 1; cl <= 8; cl *= 2) {
+      if (pass == 0 && (cl != 1 || force_cl < 0)) continue;
+      if (force_cl > 0 && cl != force_cl) continue;
+      const int rq = (c.channels + cl - 1) / cl;
+      if (rq > 255 * 16) continue;                               // packed per-thread delta counters (255 rows/thread)
+      // tensor copies: every CTA holds whole alignment classes, the rows of a CTA start at a multiple of 4 in the
+      // [beams * channels] row index, and every box lands 128-byte aligned in shared memory
+      const bool tensor = want_tensor && c.channels % (4 * cl) == 0 && strip_box_rows(rq) > 0 &&
+                          encode_tiled_fn() != nullptr;
+      const size_t smem = rfim::fd_strip_smem_bytes(rq);
+      if (smem > (pass == 1 ? half : (size_t)kMaxSmem)) continue;
+      if (pass == 0 && smem <= half) continue;                   // small tiles: two CTAs per SM (pass 1)
+      pl.cl = cl; pl.rq = rq; pl.smem = (int)smem; pl.tensor = tensor;
+      pl.box_rows = tensor ? strip_box_rows(rq) : 0;
+      pl.nw = pass == 1 ? 16 : 32;                               // one CTA per SM: twice the warps
+      return true;
+    }
+  }
+  return false;
+}
+
+int launch_fd_strip(const Call& c, const StripPlan& pl, int sms) {
+  rfim::FdStripParams P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const uint8_t*>(c.data);
+  P.dst = static_cast<uint8_t*>(c.out);
+  P.stride = c.stride;
+  P.beams = c.beams; P.C = c.channels; P.S = c.samples;
+  P.n_thr = c.n_thr;
+  for (int i = 0; i < c.n_thr; ++i) P.p[i] = quantise(c.thr[i]);
+  P.flags = c.flags;
+  P.counts = c.counts;
+  P.Rq = pl.rq;
+  P.tiles_per_beam = (c.samples + rfim::kStripCols - 1) / rfim::kStripCols;
+  P.total_tiles = (int64_t)P.tiles_per_beam * c.beams;
+  rfim::FdStripMaps maps;
+  memset(&maps, 0, sizeof(maps));
+  if (pl.tensor) {
+    if (!encode_strip_maps(c, const_cast<uint8_t*>(P.src), pl.box_rows, maps.src, P.off)) return RFIM_ERR_UNSUPPORTED;
+    P.box_rows = pl.box_rows;
+  }
+  auto kernel = pl.nw == 16 ? (pl.tensor ? rfim::fd_u8_strip_kernel<true, 16> : rfim::fd_u8_strip_kernel<false, 16>)
+                            : (pl.tensor ? rfim::fd_u8_strip_kernel<true, 32> : rfim::fd_u8_strip_kernel<false, 32>);
+  CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem));
+  cudaLaunchConfig_t cfg;
+  memset(&cfg, 0, sizeof(cfg));
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = (unsigned)pl.cl; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+  cfg.blockDim = dim3((unsigned)(32 * pl.nw), 1, 1);
+  cfg.dynamicSmemBytes = (size_t)pl.smem;
+  cfg.stream = c.stream;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  int nclusters = 0;
+  cfg.gridDim = dim3((unsigned)(sms * 2 / pl.cl * pl.cl), 1, 1);
+  CUDA_TRY(cudaOccupancyMaxActiveClusters(&nclusters, kernel, &cfg));
+  if (nclusters < 1) return RFIM_ERR_UNSUPPORTED;
+  int64_t want = P.total_tiles;
+  if (want > nclusters) want = nclusters;
+  cfg.gridDim = dim3((unsigned)(want * pl.cl), 1, 1);
+  int st = clear_outputs(c);
+  if (st != RFIM_OK) return st;
+  CUDA_TRY(cudaLaunchKernelEx(&cfg, kernel, maps, P));
+  static const char* names[2][4] = {{"fd_u8_strip1_bulk", "fd_u8_strip2_bulk", "fd_u8_strip4_bulk", "fd_u8_strip8_bulk"},
+                                    {"fd_u8_strip1", "fd_u8_strip2", "fd_u8_strip4", "fd_u8_strip8"}};
+  return after_launch(names[pl.tensor][pl.cl == 1 ? 0 : pl.cl == 2 ? 1 : pl.cl == 4 ? 2 : 3]);
+}
+
 int launch_fd_u8(const Call& c) {
   rfim::FdU8Params P;
   memset(&P, 0, sizeof(P));
@@ -344,6 +470,14 @@ int launch_fd_u8(const Call& c) {
   int st = dev_info(dv);
   if (st != RFIM_OK) return st;
 
+  if (c.variant == 0 || c.variant == 2 || c.variant == 13 || c.variant == 14) {
+    // 13: strip kernel with per-row bulk copies; 14: never the single-CTA tile (clusters, two CTAs per SM)
+    StripPlan sp;
+    if (plan_fd_u8_strip(c, c.variant != 13, c.variant == 14 ? -1 : 0, sp)) {
+      st = launch_fd_strip(c, sp, dv.sms);
+      if (st != RFIM_ERR_UNSUPPORTED) return st;
+    }
+  }
   FdPlan pl;
   int force_cl = 0, rg = 4;
   if (c.variant >= 5 && c.variant <= 8) force_cl = 1 << (c.variant - 5);

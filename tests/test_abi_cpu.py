@@ -69,7 +69,7 @@ def test_invalid_arguments_return_minus_one(fn):
     assert call(opts=ctypes.byref(o)) == -1
     o = binding.RfimOpts(); o.reserved = 1
     assert call(opts=ctypes.byref(o)) == -1
-    o = binding.RfimOpts(); o.variant = 13
+    o = binding.RfimOpts(); o.variant = 15
     assert call(opts=ctypes.byref(o)) == -1
     assert call(data=ctypes.c_void_p(0x1001), dtype=1) == -1   # float32 pointer not 4-byte aligned
     if fn == "rfim_freq_sigma_cut":

@@ -65,7 +65,7 @@ def test_config1_shape_fd(variant):
     cfg = synth.config(1)
     x = synth.fill_host(cfg)
     name, counts = check(x, [3.0], variant=variant)
-    assert name == ("fd_u8_cluster1" if variant == TILE else "fd_u8_generic")
+    assert name == ("fd_u8_strip1" if variant == TILE else "fd_u8_generic")
     _, flags, _ = oracle.freq_sigma_cut(x, [3.0])
     assert flags[0, 7].mean() > 0.9 and flags[0, 40].mean() > 0.9
 
@@ -78,7 +78,7 @@ def test_config3_arts_like_all_beams():
     synth.fill_device(cfg, x)
     x_np = x.cpu().numpy()
     name, counts = check(x_np, cfg["thresholds"], inplace=True)
-    assert name == "fd_u8_cluster8"
+    assert name == "fd_u8_strip1"
     assert all(int(c) > 0 for c in counts)
     check(x_np[:1], cfg["thresholds"], variant=GENERIC)
 
@@ -111,7 +111,7 @@ def test_shapes(C, S, variant):
         x[0, :, 0] = 77                                                                          # constant column
     name, _ = check(x, [4.0, 3.0], variant=variant)
     tiled = variant != GENERIC and S % 4 == 0
-    assert name.startswith("fd_u8_cluster") == tiled, name
+    assert name.startswith("fd_u8_strip") == tiled, name
     check(x, [3.25, 3.25, 3.25], variant=variant, inplace=True)
 
 
@@ -131,12 +131,12 @@ def test_misaligned_out():
     x[0, 3, :] = 250
     xd = torch.from_numpy(x).to(DEV)
     ref, _, _ = oracle.freq_sigma_cut(x, [3.0])
-    for shift, want in ((4, "fd_u8_generic"), (1, "fd_u8_generic"), (16, "fd_u8_cluster1")):
+    for shift, want in ((4, "fd_u8_generic"), (1, "fd_u8_generic"), (16, "fd_u8_strip1")):
         obuf = torch.zeros(16 * 1000 + 32, dtype=torch.uint8, device=DEV)
         out = obuf[shift:shift + 16000].view(1, 16, 1000)
         rfim.rfim_freq_sigma_cut(xd, [3.0], out=out)
         torch.cuda.synchronize()
-        assert rfim.rfim_last_variant() == want
+        assert rfim.rfim_last_variant().startswith(want)
         assert np.array_equal(out.cpu().numpy(), ref)
         assert int(obuf[:shift].sum()) == 0 and int(obuf[shift + 16000:].sum()) == 0
     out = obuf[4:4 + 16000].view(1, 16, 1000)
@@ -154,7 +154,7 @@ def test_unaligned_base_pointer_tile_path():
     v.copy_(torch.from_numpy(x).to(DEV))
     rfim.rfim_freq_sigma_cut(v, [4.0, 3.0])
     torch.cuda.synchronize()
-    assert rfim.rfim_last_variant().startswith("fd_u8_cluster")
+    assert rfim.rfim_last_variant().startswith("fd_u8_strip")
     ref, _, _ = oracle.freq_sigma_cut(x, [4.0, 3.0])
     assert np.array_equal(v.cpu().numpy(), ref)
     assert int(buf[:4].sum()) == 0 and int(buf[4 + 2 * 32 * 500:].sum()) == 0
@@ -207,9 +207,9 @@ def test_many_tiles_grid_wraps():
     x = noisy((40, 64, 2100), seed=71)
     x[:, 9, ::5] = 255
     name, _ = check(x, [4.0, 3.0])
-    assert name == "fd_u8_cluster1"
+    assert name == "fd_u8_strip1"
     name, _ = check(np.ascontiguousarray(x[:, :, :2096]), [4.0, 3.0])
-    assert name == "fd_u8_cluster1"
+    assert name == "fd_u8_strip1"
     for v in (CL2, CL4, CL8):
         check(x[:13], [4.0, 3.0], variant=v)
 
@@ -272,3 +272,23 @@ def test_cluster_pitch_and_phase():
         x[:, 9, :] = 200
         check(x, [4.0, 3.0], pitch=pitch, variant=CL8)
         check(x, [4.0, 3.0], pitch=pitch, variant=CL4, inplace=True)
+
+
+# ------------------------------------------------------------------------ strip kernel: cluster sizes by channel count
+@pytest.mark.parametrize("C,name", [(700, "fd_u8_strip1_bulk"), (768, "fd_u8_strip1"), (1537, "fd_u8_strip1_bulk"), (3001, "fd_u8_strip4_bulk"),
+                                    (6100, "fd_u8_strip8_bulk"), (1536, "fd_u8_strip1"), (3072, "fd_u8_strip4"),
+                                    (6144, "fd_u8_strip8"), (1028, "fd_u8_strip1_bulk")])
+def test_strip_cluster_sizes(C, name):
+    """The strip kernel splits the channels over the smallest cluster whose CTAs fit two to an SM: uneven splits,
+    a ragged last tile (S = 300 = 2 x 128 + 44), RFI channels in every CTA, empty kept intervals."""
+    x = noisy((2, C, 300), seed=C)
+    x[0, ::97, :] = 250
+    x[1, C // 2:C // 2 + 40, 17:60] = 0
+    x[1, :, 299] = 7
+    got, _ = check(x, [4.0, 3.0])
+    assert got == name
+    check(x, [0.5, 3.0, 3.0], inplace=True)
+    got, _ = check(x, [4.0, 3.0], variant=13)          # the same kernel with per-row bulk copies
+    assert got == name.replace("_bulk", "") + "_bulk"
+    got, _ = check(x, [4.0, 3.0], variant=14)          # never the whole tile in one CTA: clusters, two CTAs per SM
+    assert got.startswith("fd_u8_strip2" if C in (1536, 1537, 1028) else name.replace("_bulk", ""))
