@@ -335,6 +335,57 @@ def cpu_baseline_leg(torch, x, y, cfg, beams: int = 16):
             "gpu_output_bit_exact_on_sample": same}
 
 
+def run_table(args):
+    """--table: one JSON line per BASELINE.json config 1, 2, 3, 5 (the parity-test configurations; the bench line
+    proper is config 4).  Out of place, four rotating buffer pairs so that no repetition finds its input in L2,
+    3 warm-ups, 20 timed repetitions on CUDA events, median and best."""
+    import numpy as np
+    import torch
+
+    import paper_2001_03389_b200 as rfim
+    from paper_2001_03389_b200 import synth
+    dev = torch.device("cuda", 0)
+    peak, _ = hbm_peak()
+    cases = [(1, "time", None), (2, "time", None), (3, "freq", None), (5, "time", 256), (5, "time", 1024),
+             (5, "time", 12500)]
+    for (n, op, window) in cases:
+        cfg = synth.config(n)
+        host = synth.fill_host(cfg) if cfg["dtype"] == "f32" or cfg["beams"] * cfg["channels"] < 4096 else None
+        pairs = []
+        for _ in range(4):
+            if host is not None:
+                x = torch.from_numpy(host).to(dev)
+            else:
+                x = torch.empty((cfg["beams"], cfg["channels"], cfg["samples"]), dtype=torch.uint8, device=dev)
+                synth.fill_device(cfg, x)
+            pairs.append((x, torch.empty_like(x)))
+        ks = cfg["thresholds"]
+
+        def call(i):
+            x, y = pairs[i % 4]
+            if op == "time":
+                rfim.rfim_time_sigma_cut(x, ks, cfg["policy"], out=y, window=window or 0)
+            else:
+                rfim.rfim_freq_sigma_cut(x, ks, cfg["policy"], out=y)
+        for i in range(3):
+            call(i)
+        torch.cuda.synchronize()
+        ms = []
+        for i in range(20):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(); call(i); e1.record(); torch.cuda.synchronize()
+            ms.append(e0.elapsed_time(e1))
+        med, best = float(np.median(ms)), float(min(ms))
+        nbytes = 2 * pairs[0][0].numel() * pairs[0][0].element_size()
+        print(json.dumps({"config": n, "op": op, "window": window, "kernel": rfim.rfim_last_variant(),
+                          "thresholds": ks, "policy": cfg["policy"], "ms_median": med, "ms_best": best,
+                          "samples_per_s": pairs[0][0].numel() / (med * 1e-3), "GBps_rw": nbytes / (med * 1e-3) / 1e9,
+                          "frac_of_measured_peak": nbytes / (med * 1e-3) / 1e9 / peak,
+                          "frac_of_nominal_8000": nbytes / (med * 1e-3) / 1e9 / 8000.0,
+                          "realtime_margin": BATCH_SECONDS / (med * 1e-3)}), flush=True)
+        del pairs
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -344,13 +395,16 @@ def main():
     ap.add_argument("--beams", type=int, default=0, help="override the beam count (testing only)")
     ap.add_argument("--td-variant", type=int, default=0, help="kernel variant for TDSC (tuning only; 0 = auto)")
     ap.add_argument("--fd-variant", type=int, default=0, help="kernel variant for FDSC (tuning only; 0 = auto)")
+    ap.add_argument("--table", action="store_true", help="time configs 1, 2, 3, 5 instead (one JSON line each)")
     ap.add_argument("--no-cpu-baseline", action="store_true", help="skip the oracle leg (profiling runs)")
     ap.add_argument("--no-e2e", action="store_true", help="skip the host-buffer leg (profiling runs)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     from paper_2001_03389_b200 import synth
     cfg = synth.config(4, **({"beams": args.beams} if args.beams else {}))
-    if args.impl == "reference":
+    if args.table:
+        run_table(args)
+    elif args.impl == "reference":
         run_reference(args, cfg)
     else:
         run_ours(args, cfg)
