@@ -9,6 +9,7 @@
 
 #include "common.cuh"
 #include "fd_u8.cuh"
+#include "fd_u8_binned.cuh"
 #include "fd_u8_strip.cuh"
 #include "td_f32.cuh"
 #include "td_u8.cuh"
@@ -469,6 +470,23 @@ int launch_fd_u8(const Call& c) {
   DevInfo dv;
   int st = dev_info(dv);
   if (st != RFIM_OK) return st;
+
+  if (c.bin_size != c.channels) {                                  // per-bin mean correction: correctness path
+    if (c.policy != RFIM_REPLACE_MEAN || c.variant >= 2) return RFIM_ERR_UNSUPPORTED;
+    rfim::FdBinnedParams B;
+    memset(&B, 0, sizeof(B));
+    B.src = P.src; B.dst = P.dst; B.stride = c.stride;
+    B.beams = c.beams; B.C = c.channels; B.S = c.samples; B.nb = c.bin_size;
+    B.n_thr = c.n_thr;
+    for (int i = 0; i < c.n_thr; ++i) B.p[i] = P.p[i];
+    B.flags = c.flags; B.counts = c.counts;
+    const int64_t ncol = (int64_t)c.beams * c.samples;
+    int64_t grid = (ncol + rfim::kFdBinnedThreads - 1) / rfim::kFdBinnedThreads;
+    if (grid > (int64_t)dv.sms * 16) grid = (int64_t)dv.sms * 16;
+    if ((st = clear_outputs(c)) != RFIM_OK) return st;
+    rfim::fd_u8_binned_kernel<<<(unsigned)grid, rfim::kFdBinnedThreads, 0, c.stream>>>(B);
+    return after_launch("fd_u8_binned_generic");
+  }
 
   if (c.variant == 0 || c.variant == 2 || c.variant == 13 || c.variant == 14) {
     // 13: strip kernel with per-row bulk copies; 14: never the single-CTA tile (clusters, two CTAs per SM)
