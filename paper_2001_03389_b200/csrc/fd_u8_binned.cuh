@@ -20,6 +20,7 @@ struct FdBinnedParams {
   int64_t stride;
   int beams, C, S, nb;
   int n_thr;
+  int policy;                   // 0 = bin mean (rounded half up), 1 = lower median of the bin
   uint32_t p[16];
   uint8_t* flags;
   unsigned long long* counts;
@@ -58,7 +59,20 @@ __global__ void __launch_bounds__(kFdBinnedThreads) fd_u8_binned_kernel(const Fd
         for (int bin = 0; bin < nbins; ++bin) {
           uint64_t Sb = 0;
           for (int j = 0; j < P.nb; ++j) Sb += dst[(int64_t)(bin * P.nb + j) * P.stride];
-          const uint32_t r = (uint32_t)((2 * Sb + (uint64_t)P.nb) / (2 * (uint64_t)P.nb));
+          uint32_t r = (uint32_t)((2 * Sb + (uint64_t)P.nb) / (2 * (uint64_t)P.nb));
+          if (P.policy == 1) {
+            // lower median (rank (nb - 1) / 2) of the bin's snapshot: smallest v with #{x <= v} > rank, by
+            // bisection on the byte value with counting passes (8 passes; correctness path)
+            const uint32_t rank = (uint32_t)(P.nb - 1) >> 1;
+            uint32_t lo_v = 0, hi_v = 255;
+            while (lo_v < hi_v) {
+              const uint32_t mid = (lo_v + hi_v) >> 1;
+              uint32_t le = 0;
+              for (int j = 0; j < P.nb; ++j) le += dst[(int64_t)(bin * P.nb + j) * P.stride] <= mid;
+              if (le > rank) hi_v = mid; else lo_v = mid + 1;
+            }
+            r = lo_v;
+          }
           for (int j = 0; j < P.nb; ++j) {
             const int c = bin * P.nb + j;
             const uint32_t x = dst[(int64_t)c * P.stride];

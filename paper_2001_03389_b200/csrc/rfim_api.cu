@@ -9,6 +9,7 @@
 
 #include "common.cuh"
 #include "fd_u8.cuh"
+#include "fd_f32.cuh"
 #include "fd_u8_binned.cuh"
 #include "fd_u8_strip.cuh"
 #include "td_f32.cuh"
@@ -471,13 +472,14 @@ int launch_fd_u8(const Call& c) {
   int st = dev_info(dv);
   if (st != RFIM_OK) return st;
 
-  if (c.bin_size != c.channels) {                                  // per-bin mean correction: correctness path
-    if (c.policy != RFIM_REPLACE_MEAN || c.variant >= 2) return RFIM_ERR_UNSUPPORTED;
+  if (c.bin_size != c.channels || c.policy == RFIM_REPLACE_MEDIAN) {   // per-bin mean correction and / or median
+    if (c.variant >= 2) return RFIM_ERR_UNSUPPORTED;                    // replacement: correctness path
     rfim::FdBinnedParams B;
     memset(&B, 0, sizeof(B));
     B.src = P.src; B.dst = P.dst; B.stride = c.stride;
     B.beams = c.beams; B.C = c.channels; B.S = c.samples; B.nb = c.bin_size;
     B.n_thr = c.n_thr;
+    B.policy = (int)c.policy;
     for (int i = 0; i < c.n_thr; ++i) B.p[i] = P.p[i];
     B.flags = c.flags; B.counts = c.counts;
     const int64_t ncol = (int64_t)c.beams * c.samples;
@@ -527,6 +529,31 @@ int launch_fd_u8(const Call& c) {
   return after_launch("fd_u8_generic");
 }
 
+// ------------------------------------------------------------------------------------------ FD f32
+int launch_fd_f32(const Call& c) {
+  rfim::FdF32Params P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const float*>(c.data);
+  P.dst = static_cast<float*>(c.out);
+  P.stride = c.stride;
+  P.beams = c.beams; P.C = c.channels; P.S = c.samples; P.nb = c.bin_size;
+  P.n_thr = c.n_thr;
+  P.policy = (int)c.policy;
+  for (int i = 0; i < c.n_thr; ++i) P.k[i] = c.thr[i];
+  P.flags = c.flags;
+  P.counts = c.counts;
+  if (c.variant >= 2) return RFIM_ERR_UNSUPPORTED;                 // only the correctness path exists
+  DevInfo dv;
+  int st = dev_info(dv);
+  if (st != RFIM_OK) return st;
+  const int64_t ncol = (int64_t)c.beams * c.samples;
+  int64_t grid = (ncol + rfim::kFdF32Threads - 1) / rfim::kFdF32Threads;
+  if (grid > (int64_t)dv.sms * 16) grid = (int64_t)dv.sms * 16;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  rfim::fd_f32_generic_kernel<<<(unsigned)grid, rfim::kFdF32Threads, 0, c.stream>>>(P);
+  return after_launch("fd_f32_generic");
+}
+
 }  // namespace
 
 // =============================================================================================
@@ -557,7 +584,7 @@ int rfim_freq_sigma_cut(void* data, int beams, int channels, int samples, rfim_d
     return copy_through(c);
   }
   if (dtype == RFIM_U8) return launch_fd_u8(c);
-  return RFIM_ERR_UNSUPPORTED;
+  return launch_fd_f32(c);
 }
 
 int rfim_sigma_cut_host(void* data, void* out, int beams, int channels, int samples, rfim_dtype dtype,

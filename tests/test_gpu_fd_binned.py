@@ -69,8 +69,46 @@ def test_binned_config3_shape_fig5_parameters():
     check(x, [2.75, 2.75, 2.75], 32, pitch=512)
 
 
-def test_binned_median_is_unsupported():
-    x = torch.zeros((1, 64, 128), dtype=torch.uint8, device=DEV)
-    with pytest.raises(rfim.RfimError) as e:
-        rfim.rfim_freq_sigma_cut(x, [3.0], policy="median", bin_size=32)
-    assert e.value.status == -2
+def check_policy(x_np, ks, bin_size, policy):
+    pol = oracle.MEDIAN if policy == "median" else oracle.MEAN
+    ref, rflags, rcounts = oracle.freq_sigma_cut(x_np, ks, policy=pol, bin_size=bin_size)
+    x = torch.from_numpy(x_np).to(DEV)
+    flags = torch.zeros(x_np.shape, dtype=torch.uint8, device=DEV)
+    counts = torch.zeros(len(ks), dtype=torch.int64, device=DEV)
+    out = torch.empty_like(x)
+    rfim.rfim_freq_sigma_cut(x, ks, policy, out=out, bin_size=bin_size, flags=flags, counts=counts)
+    torch.cuda.synchronize()
+    got = out.cpu().numpy()
+    if x_np.dtype == np.uint8:
+        assert np.array_equal(got, ref)
+    else:
+        # same fp64 operations in the same order as the definition: identical flags, values within 1e-5 relative
+        assert np.allclose(got, ref, rtol=1e-5, atol=0.0)
+    assert np.array_equal(flags.cpu().numpy(), rflags)
+    assert counts.cpu().tolist() == [int(c) for c in rcounts]
+    return rfim.rfim_last_variant(), rcounts
+
+
+@pytest.mark.parametrize("C,S,nb", [(64, 100, 0), (64, 37, 32), (96, 20, 8), (33, 50, 0), (20, 16, 1)])
+def test_median_replacement_u8(C, S, nb):
+    """FDSC with the median strategy: the test still uses mean and sigma, the
+    replacement is the lower median of the bin."""
+    x = banded((2, C, S), seed=C + S + nb)
+    name, counts = check_policy(x, [3.0, 3.0], nb, "median")
+    assert name == "fd_u8_binned_generic"
+    check_policy(x, [1.0], nb, "median")
+
+
+@pytest.mark.parametrize("policy", ["mean", "median"])
+@pytest.mark.parametrize("C,S,nb", [(64, 100, 0), (64, 37, 32), (96, 20, 8), (1536, 24, 32)])
+def test_float32_fdsc(C, S, nb, policy):
+    """float32 FDSC, one bin or bins, mean or median."""
+    rng = np.random.default_rng(C * 5 + S + nb)
+    band = 3.0 * rng.random((2, (C + 31) // 32, 1)).repeat(32, axis=1)[:, :C]
+    x = rng.normal(band, 1.0, (2, C, S))
+    x[0, C // 3, :] += 8.0
+    x[:, :, S // 2] += 10.0
+    x = x.astype(np.float32)
+    name, counts = check_policy(x, [2.75, 2.75], nb, policy)
+    assert name == "fd_f32_generic" and int(counts[0]) > 0
+    check_policy(x, [4.0, 3.0, 2.0], nb, policy)
