@@ -325,18 +325,27 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
       // inside the sweep would make every lane pay for it at every step.
       {
         uint32_t* col = col0;
-        unsigned long long hm = 0ull;
-        int i = 0;
-#pragma unroll 4
-        for (; i + 4 <= ni; i += 4, col += 4 * RS) {
-          const uint32_t w0 = col[0], w1 = col[RS], w2 = col[2 * RS], w3 = col[3 * RS];
+        auto step_hits = [&](const uint32_t* c) {        // packed test of four rows of this thread's word column
+          const uint32_t w0 = c[0], w1 = c[RS], w2 = c[2 * RS], w3 = c[3 * RS];
           uint32_t aO = __viaddmax_u16x2(w0, negO, 0u), aE = __viaddmax_u16x2(w0 << 8, negE, 0u);
           uint32_t bO = __viaddmax_u16x2(w1, negO, 0u), bE = __viaddmax_u16x2(w1 << 8, negE, 0u);
           aO = __viaddmax_u16x2(w2, negO, aO); aE = __viaddmax_u16x2(w2 << 8, negE, aE);
           bO = __viaddmax_u16x2(w3, negO, bO); bE = __viaddmax_u16x2(w3 << 8, negE, bE);
           aO = __vimax3_u16x2(aO, bO, thrO); aE = __vimax3_u16x2(aE, bE, thrE);
-          if (aO != thrO || aE != thrE) hm |= 1ull << (i >> 2);
-        }
+          return ((aO ^ thrO) | (aE ^ thrE)) != 0u;
+        };
+        // one bit per step in two 32-bit words (a running bit instead of a 64-bit variable shift per step)
+        const int n4 = ni >> 2, nA = min(n4, 32);
+        uint32_t hm0 = 0u, hm1 = 0u, bit = 1u;
+        int st4 = 0;
+#pragma unroll 4
+        for (; st4 < nA; ++st4, col += 4 * RS, bit <<= 1)
+          if (step_hits(col)) hm0 |= bit;
+        bit = 1u;
+        for (; st4 < n4; ++st4, col += 4 * RS, bit <<= 1)
+          if (step_hits(col)) hm1 |= bit;
+        unsigned long long hm = ((unsigned long long)hm1 << 32) | hm0;
+        int i = 4 * n4;
         for (; i < ni; ++i, col += RS) fix_word(col, col[0], i);
         const int nsteps = ni >> 2;
         if (slow) hm = nsteps < 64 ? (1ull << nsteps) - 1ull : ~0ull;
