@@ -283,6 +283,11 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
     }
     if (P.n_thr > 0) exchange(true, 0);
 
+    // Tensor path, full-width tile: the LAST sweep writes the rows it finds clean straight from its registers
+    // (F6 fused into F4: no second pass over shared memory for them); repaired rows are written by the repair.
+    bool fused_store = false;
+    uint8_t* const gds0 = P.dst + ((int64_t)b * C + c0 + warp) * P.stride + s0 + 4 * lane;
+    const int64_t rstep = (int64_t)kStripWarps * P.stride;          // bytes between consecutive rows of this thread
     // ------------------------------------------------------------------ F3..F5: thresholds, on chip
     for (int it = 0; it < P.n_thr; ++it) {
       const uint4 ck = K->chk[lane];
@@ -338,15 +343,46 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
         const int n4 = ni >> 2, nA = min(n4, 32);
         uint32_t hm0 = 0u, hm1 = 0u, bit = 1u;
         int st4 = 0;
+        const bool fuse = kTensor && !need_stats && tw == kStripCols;
+        if (fuse) {
+          fused_store = true;
+          auto step_store = [&](const uint32_t* c, uint8_t* g) {   // the same test; clean rows go out at once
+            const uint32_t w0 = c[0], w1 = c[RS], w2 = c[2 * RS], w3 = c[3 * RS];
+            uint32_t aO = __viaddmax_u16x2(w0, negO, 0u), aE = __viaddmax_u16x2(w0 << 8, negE, 0u);
+            uint32_t bO = __viaddmax_u16x2(w1, negO, 0u), bE = __viaddmax_u16x2(w1 << 8, negE, 0u);
+            aO = __viaddmax_u16x2(w2, negO, aO); aE = __viaddmax_u16x2(w2 << 8, negE, aE);
+            bO = __viaddmax_u16x2(w3, negO, bO); bE = __viaddmax_u16x2(w3 << 8, negE, bE);
+            aO = __vimax3_u16x2(aO, bO, thrO); aE = __vimax3_u16x2(aE, bE, thrE);
+            const bool h = ((aO ^ thrO) | (aE ^ thrE)) != 0u;
+            if (!h) {
+              *reinterpret_cast<uint32_t*>(g) = w0;
+              *reinterpret_cast<uint32_t*>(g + rstep) = w1;
+              *reinterpret_cast<uint32_t*>(g + 2 * rstep) = w2;
+              *reinterpret_cast<uint32_t*>(g + 3 * rstep) = w3;
+            }
+            return h;
+          };
+          uint8_t* g = gds0;
+#pragma unroll 2
+          for (; st4 < nA; ++st4, col += 4 * RS, g += 4 * rstep, bit <<= 1)
+            if (step_store(col, g)) hm0 |= bit;
+          bit = 1u;
+          for (; st4 < n4; ++st4, col += 4 * RS, g += 4 * rstep, bit <<= 1)
+            if (step_store(col, g)) hm1 |= bit;
+        } else {
 #pragma unroll 4
-        for (; st4 < nA; ++st4, col += 4 * RS, bit <<= 1)
-          if (step_hits(col)) hm0 |= bit;
-        bit = 1u;
-        for (; st4 < n4; ++st4, col += 4 * RS, bit <<= 1)
-          if (step_hits(col)) hm1 |= bit;
+          for (; st4 < nA; ++st4, col += 4 * RS, bit <<= 1)
+            if (step_hits(col)) hm0 |= bit;
+          bit = 1u;
+          for (; st4 < n4; ++st4, col += 4 * RS, bit <<= 1)
+            if (step_hits(col)) hm1 |= bit;
+        }
         unsigned long long hm = ((unsigned long long)hm1 << 32) | hm0;
         int i = 4 * n4;
-        for (; i < ni; ++i, col += RS) fix_word(col, col[0], i);
+        for (; i < ni; ++i, col += RS) {
+          fix_word(col, col[0], i);
+          if (fuse) *reinterpret_cast<uint32_t*>(gds0 + (int64_t)i * rstep) = col[0];
+        }
         const int nsteps = ni >> 2;
         if (slow) hm = nsteps < 64 ? (1ull << nsteps) - 1ull : ~0ull;
         while (hm) {
@@ -358,6 +394,13 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
           if (hit(w1)) fix_word(c4 + RS, w1, 4 * st + 1);
           if (hit(w2)) fix_word(c4 + 2 * RS, w2, 4 * st + 2);
           if (hit(w3)) fix_word(c4 + 3 * RS, w3, 4 * st + 3);
+          if (fuse) {
+            uint8_t* g = gds0 + (int64_t)st * 4 * rstep;
+            *reinterpret_cast<uint32_t*>(g) = c4[0];
+            *reinterpret_cast<uint32_t*>(g + rstep) = c4[RS];
+            *reinterpret_cast<uint32_t*>(g + 2 * rstep) = c4[2 * RS];
+            *reinterpret_cast<uint32_t*>(g + 3 * rstep) = c4[3 * RS];
+          }
         }
       }
       if ((need_stats || P.counts) && __any_sync(FULL, cnt4 != 0u)) {
@@ -388,7 +431,7 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
       // ever touched its rows, so no barrier is needed before the store.
       uint8_t* gd = P.dst + ((int64_t)b * C + c0 + warp) * P.stride + s0 + 4 * lane;
       const uint32_t* col = col0;
-      const int nb = tw - 4 * lane;                 // valid bytes of this lane's word
+      const int nb = fused_store ? 0 : tw - 4 * lane;   // valid bytes of this lane's word (0: already written)
       if (nb >= 4) {
 #pragma unroll 4
         for (int i = 0; i < ni; ++i, col += RS, gd += (int64_t)kStripWarps * P.stride)
