@@ -89,7 +89,7 @@ struct __align__(16) FdStripCtrl {
   uint32_t acc[2][2 * kStripCols];               // [buffer][S of 128 columns, Q of 128 columns]
   uint4 chk[kStripWords];                        // per word column {negE, negO, thrE, thrO}
   uint8_t lo[kStripCols], hi[kStripCols], rr[kStripCols];
-  uint64_t bar[4];                               // tensor path: one per alignment class; bulk path: bar[0]
+  uint64_t bar[32];                              // tensor path: one per alignment class, or one per warp (kWarpBox); bulk path: bar[0]
 };
 __host__ __device__ inline size_t fd_strip_smem_bytes(int Rq) {
   return (size_t)Rq * kStripPitchW * 4 + sizeof(FdStripCtrl);
@@ -105,8 +105,11 @@ __device__ __forceinline__ void smem_red_add(uint32_t* p, uint32_t v) {
   asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(smem_addr(p)), "r"(v) : "memory");
 }
 
-// NW warps per CTA: 16 (two CTAs per SM) or 32 (one CTA per SM holding a whole tile)
-template <bool kTensor, int NW>
+// NW warps per CTA: 16 (two CTAs per SM) or 32 (one CTA per SM holding a whole tile).
+// kWarpBox (tensor path, Rq a multiple of 8 NW): a warp owns Rq / NW CONSECUTIVE rows of its alignment class, one
+// tensor box with its own mbarrier, so every warp runs its own copy-in / store / next-copy-in pipeline and no warp
+// waits for the slowest warp of its class before the next tile's rows are requested.
+template <bool kTensor, int NW, bool kWarpBox>
 __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(const __grid_constant__ FdStripMaps maps,
                                                                                 const FdStripParams P) {
   constexpr int kStripThreads = 32 * NW, kStripWarps = NW;
@@ -114,7 +117,7 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
   constexpr int PW = kStripPitchW;
   // words between consecutive rows (16 apart) of one thread.  Tensor path: the rows of alignment class k are
   // stored together (class-major), local row r at shared-memory row (r & 3) * Rq / 4 + (r >> 2).
-  constexpr int RS = kTensor ? (NW / 4) * PW : kStripWarps * PW;
+  constexpr int RS = kWarpBox ? PW : kTensor ? (NW / 4) * PW : kStripWarps * PW;
   const int C = P.C, Rq = P.Rq;
   uint32_t* tile = reinterpret_cast<uint32_t*>(smem);
   FdStripCtrl* K = reinterpret_cast<FdStripCtrl*>(smem + (size_t)Rq * PW * 4);
@@ -122,7 +125,10 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
   const uint32_t rank = cluster_ctarank(), ncta = cluster_nctarank();
   const int c0 = (int)rank * Rq;                      // first channel of this CTA
   const int nrows = max(0, min(Rq, C - c0));
-  const int ni = nrows > warp ? (nrows - warp + kStripWarps - 1) / kStripWarps : 0;   // rows warp + 16 i
+  const int ni = kWarpBox ? Rq / NW : nrows > warp ? (nrows - warp + kStripWarps - 1) / kStripWarps : 0;   // rows of this thread
+  // logical row (channel - c0) of this thread's i-th row: row0 + rowmul * i
+  const int row0 = kWarpBox ? 4 * ((warp >> 2) * ni) + (warp & 3) : warp;
+  constexpr int rowmul = kWarpBox ? 4 : kStripWarps;
   const int cpc = kStripCols / (int)ncta;             // columns owned per CTA (F3)
   const bool owner = tid < cpc;
   const int ocol = (int)rank * cpc + tid;
@@ -132,7 +138,7 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
   if (tid == 0) {
     if (kTensor) {
 #pragma unroll
-      for (int k = 0; k < 4; ++k) mbar_init(&K->bar[k], 1);
+      for (int k = 0; k < (kWarpBox ? NW : 4); ++k) mbar_init(&K->bar[k], 1);
     } else {
       mbar_init(&K->bar[0], nload > 0 ? nload : 1);
     }
@@ -158,8 +164,20 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
     for (int y = 0; y < (Rq >> 2); y += P.box_rows)
       tma_load_2d(tile + ((size_t)k * (Rq >> 2) + y) * PW, &maps.src[k], s0, ycls + y, &K->bar[k]);
   };
+  auto issue_warp_load = [&](int64_t t) {             // lane 0 of every warp: the warp's own box
+    const int b = (int)(t / P.tiles_per_beam);
+    const int s0 = (int)(t % P.tiles_per_beam) * kStripCols;
+    const int ycls = (int)(((int64_t)b * C + c0) >> 2);
+    mbar_arrive_expect_tx(&K->bar[warp], (uint32_t)ni * PW * 4u);
+    tma_load_2d(tile + ((size_t)cls * (Rq >> 2) + (size_t)(warp >> 2) * ni) * PW, &maps.src[cls], s0,
+                ycls + (warp >> 2) * ni, &K->bar[warp]);
+  };
   const uint32_t nclusters = cluster_nid_x();
-  if (kTensor && tid < 4 && (int64_t)cluster_id_x() < P.total_tiles) issue_class_load(cluster_id_x(), tid);
+  if (kWarpBox) {
+    if (lane == 0 && (int64_t)cluster_id_x() < P.total_tiles) issue_warp_load(cluster_id_x());
+  } else if (kTensor && tid < 4 && (int64_t)cluster_id_x() < P.total_tiles) {
+    issue_class_load(cluster_id_x(), tid);
+  }
 
   uint32_t phase = 0;
   int buf = 0;                                        // accumulator buffer of the next exchange
@@ -187,7 +205,7 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
         bulk_load(tile + (size_t)r * PW, g - off, (off + (uint32_t)tw + 15u) & ~15u, &K->bar[0]);
       }
     }
-    mbar_wait(&K->bar[kTensor ? cls : 0], phase);
+    mbar_wait(&K->bar[kWarpBox ? warp : kTensor ? cls : 0], phase);
     phase ^= 1;
     // While this tile is being processed, HBM delivers the NEXT tile into L2: the copies issued after this
     // tile's stores then come from L2 instead of waiting for DRAM behind those stores (6.6 -> 5.9 ms on config 4;
@@ -202,8 +220,10 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
 
     // rows warp + 16 i share the 16-byte phase of their global address: word offset of column s0 in them
     const int offw = (int)((reinterpret_cast<uintptr_t>(gsrc + (int64_t)warp * P.stride) & 15) >> 2);
-    uint32_t* const col0 = kTensor ? tile + ((size_t)(warp & 3) * (Rq >> 2) + (warp >> 2)) * PW + (P.off[warp & 3] >> 2) + lane
-                                   : tile + (size_t)warp * PW + offw + lane;
+    uint32_t* const col0 =
+        kWarpBox ? tile + ((size_t)cls * (Rq >> 2) + (size_t)(warp >> 2) * ni) * PW + (P.off[cls] >> 2) + lane
+        : kTensor ? tile + ((size_t)cls * (Rq >> 2) + (warp >> 2)) * PW + (P.off[cls] >> 2) + lane
+                  : tile + (size_t)warp * PW + offw + lane;
 
     // one exchange: accumulators of all CTAs -> owners -> (lo, hi, r, packed constants) in every CTA
     auto exchange = [&](bool first, int itn) {
@@ -286,8 +306,8 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
     // Tensor path, full-width tile: the LAST sweep writes the rows it finds clean straight from its registers
     // (F6 fused into F4: no second pass over shared memory for them); repaired rows are written by the repair.
     bool fused_store = false;
-    uint8_t* const gds0 = P.dst + ((int64_t)b * C + c0 + warp) * P.stride + s0 + 4 * lane;
-    const int64_t rstep = (int64_t)kStripWarps * P.stride;          // bytes between consecutive rows of this thread
+    uint8_t* const gds0 = P.dst + ((int64_t)b * C + c0 + row0) * P.stride + s0 + 4 * lane;
+    const int64_t rstep = (int64_t)rowmul * P.stride;               // bytes between consecutive rows of this thread
     // ------------------------------------------------------------------ F3..F5: thresholds, on chip
     for (int it = 0; it < P.n_thr; ++it) {
       const uint4 ck = K->chk[lane];
@@ -316,7 +336,7 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
         sq[2] = __dp4a(f & 0x00ff0000u, f, sq[2]);
         sq[3] = __dp4a(f & 0xff000000u, f, sq[3]);
         if (P.flags) {
-          uint8_t* fl = P.flags + ((int64_t)b * C + c0 + warp + kStripWarps * i) * P.S + s0 + 4 * lane;
+          uint8_t* fl = P.flags + ((int64_t)b * C + c0 + row0 + rowmul * i) * P.S + s0 + 4 * lane;
 #pragma unroll
           for (int u = 0; u < 4; ++u)
             if ((m >> (8 * u)) & 1u) fl[u] = 1;
@@ -429,23 +449,28 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
     if (kTensor) {
       // a warp writes the 128-byte segment of one row per step: 32 lanes x one 32-bit word.  Only this warp
       // ever touched its rows, so no barrier is needed before the store.
-      uint8_t* gd = P.dst + ((int64_t)b * C + c0 + warp) * P.stride + s0 + 4 * lane;
+      uint8_t* gd = gds0;
       const uint32_t* col = col0;
       const int nb = fused_store ? 0 : tw - 4 * lane;   // valid bytes of this lane's word (0: already written)
       if (nb >= 4) {
 #pragma unroll 4
-        for (int i = 0; i < ni; ++i, col += RS, gd += (int64_t)kStripWarps * P.stride)
+        for (int i = 0; i < ni; ++i, col += RS, gd += rstep)
           *reinterpret_cast<uint32_t*>(gd) = col[0];
       } else if (nb > 0) {
-        for (int i = 0; i < ni; ++i, col += RS, gd += (int64_t)kStripWarps * P.stride) {
+        for (int i = 0; i < ni; ++i, col += RS, gd += rstep) {
           const uint32_t w = col[0];
           for (int u = 0; u < nb; ++u) gd[u] = (uint8_t)(w >> (8 * u));
         }
       }
       // the class's rows are free once its NW / 4 warps are here: fetch the class's rows of the next tile
       fence_proxy_async_smem();
-      asm volatile("bar.sync %0, %1;" ::"r"(1 + cls), "n"(32 * (NW / 4)) : "memory");
-      if (warp == cls && lane == 0 && t + nclusters < P.total_tiles) issue_class_load(t + nclusters, cls);
+      if (kWarpBox) {                               // the warp's rows are free: fetch its rows of the next tile
+        __syncwarp();
+        if (lane == 0 && t + nclusters < P.total_tiles) issue_warp_load(t + nclusters);
+      } else {
+        asm volatile("bar.sync %0, %1;" ::"r"(1 + cls), "n"(32 * (NW / 4)) : "memory");
+        if (warp == cls && lane == 0 && t + nclusters < P.total_tiles) issue_class_load(t + nclusters, cls);
+      }
     } else {
       fence_proxy_async_smem();                     // generic-proxy writes of the repair -> async proxy
       __syncthreads();

@@ -369,7 +369,7 @@ bool encode_strip_maps(const Call& c, uint8_t* base, int box_rows, CUtensorMap* 
   return true;
 }
 
-struct StripPlan { int cl, rq, smem, box_rows, nw; bool tensor; };
+struct StripPlan { int cl, rq, smem, box_rows, nw; bool tensor, warp_box; };
 // rows per tensor copy: divides the Rq / 4 rows of a class, at most 256, and every box lands 128-byte aligned
 int strip_box_rows(int rq) {
   const int rc = rq / 4;
@@ -403,6 +403,9 @@ bool plan_fd_u8_strip(const Call& c, bool want_tensor, int force_cl, StripPlan& 
       pl.cl = cl; pl.rq = rq; pl.smem = (int)smem; pl.tensor = tensor;
       pl.box_rows = tensor ? strip_box_rows(rq) : 0;
       pl.nw = pass == 1 ? 16 : 32;                               // one CTA per SM: twice the warps
+      // one box per warp: Rq / nw consecutive class rows each, 128-byte aligned in shared memory, at most 256
+      pl.warp_box = tensor && pl.nw == 32 && rq % (8 * pl.nw) == 0 && rq / pl.nw <= 256;
+      if (pl.warp_box) pl.box_rows = rq / pl.nw;
       return true;
     }
   }
@@ -429,8 +432,9 @@ int launch_fd_strip(const Call& c, const StripPlan& pl, int sms) {
     if (!encode_strip_maps(c, const_cast<uint8_t*>(P.src), pl.box_rows, maps.src, P.off)) return RFIM_ERR_UNSUPPORTED;
     P.box_rows = pl.box_rows;
   }
-  auto kernel = pl.nw == 16 ? (pl.tensor ? rfim::fd_u8_strip_kernel<true, 16> : rfim::fd_u8_strip_kernel<false, 16>)
-                            : (pl.tensor ? rfim::fd_u8_strip_kernel<true, 32> : rfim::fd_u8_strip_kernel<false, 32>);
+  auto kernel = pl.nw == 16 ? (pl.tensor ? rfim::fd_u8_strip_kernel<true, 16, false> : rfim::fd_u8_strip_kernel<false, 16, false>)
+                : pl.warp_box ? rfim::fd_u8_strip_kernel<true, 32, true>
+                              : (pl.tensor ? rfim::fd_u8_strip_kernel<true, 32, false> : rfim::fd_u8_strip_kernel<false, 32, false>);
   CUDA_TRY(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, pl.smem));
   cudaLaunchConfig_t cfg;
   memset(&cfg, 0, sizeof(cfg));

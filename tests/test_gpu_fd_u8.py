@@ -277,7 +277,8 @@ def test_cluster_pitch_and_phase():
 # ------------------------------------------------------------------------ strip kernel: cluster sizes by channel count
 @pytest.mark.parametrize("C,name", [(700, "fd_u8_strip1_bulk"), (768, "fd_u8_strip1"), (1537, "fd_u8_strip1_bulk"), (3001, "fd_u8_strip4_bulk"),
                                     (6100, "fd_u8_strip8_bulk"), (1536, "fd_u8_strip1"), (3072, "fd_u8_strip4"),
-                                    (6144, "fd_u8_strip8"), (1028, "fd_u8_strip1_bulk")])
+                                    (6144, "fd_u8_strip8"), (1028, "fd_u8_strip1_bulk"), (1024, "fd_u8_strip1"),
+                                    (1280, "fd_u8_strip1"), (1152, "fd_u8_strip1")])
 def test_strip_cluster_sizes(C, name):
     """The strip kernel splits the channels over the smallest cluster whose CTAs fit two to an SM: uneven splits,
     a ragged last tile (S = 300 = 2 x 128 + 44), RFI channels in every CTA, empty kept intervals."""
@@ -291,4 +292,4 @@ def test_strip_cluster_sizes(C, name):
     got, _ = check(x, [4.0, 3.0], variant=13)          # the same kernel with per-row bulk copies
     assert got == name.replace("_bulk", "") + "_bulk"
     got, _ = check(x, [4.0, 3.0], variant=14)          # never the whole tile in one CTA: clusters, two CTAs per SM
-    assert got.startswith("fd_u8_strip2" if C in (1536, 1537, 1028) else name.replace("_bulk", ""))
+    assert got.startswith("fd_u8_strip2" if C in (1536, 1537, 1028, 1024, 1280, 1152) else name.replace("_bulk", ""))
