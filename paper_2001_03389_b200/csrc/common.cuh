@@ -115,6 +115,34 @@ __device__ __forceinline__ void thread_bounds_u8_sqrt(const U8Cut& c, int& lo, i
   if (lo > hi) { lo = 1; hi = 0; }
 }
 
+// The same closed form with 32-bit quotients: floor(a / n) for a < 2^32 from inv = ceil(2^32 / n) is
+// umulhi(a, inv) or one less (a inv / 2^32 < a / n + 1), so one exact check finishes it.  Used where n is the
+// same for every column (FDSC: n = channels) and the host passes inv.
+__device__ __forceinline__ uint32_t div_floor_u32(uint32_t a, uint32_t n, uint32_t inv) {
+  uint32_t q = __umulhi(a, inv);
+  if ((uint64_t)q * n > a) --q;
+  return q;
+}
+// requires 2 <= n and S + T < 2^32 (else the caller uses thread_bounds_u8_sqrt); r = rounded mean floor((2S+n)/(2n))
+__device__ __forceinline__ void thread_bounds_u8_sqrt32(const U8Cut& c, uint32_t inv, int& lo, int& hi, uint32_t& r) {
+  const uint32_t S = c.S, N = c.N;
+  r = div_floor_u32(S + (N >> 1), N, inv);                     // floor((2S+N)/(2N)) = floor((S + floor(N/2)) / N) for even N;
+  if (N & 1u) {                                                // odd N: compare 2 (S - r N) + N with 2 N exactly
+    const uint32_t rem2 = 2u * (S - div_floor_u32(S, N, inv) * N) + N;
+    r = div_floor_u32(S, N, inv) + (rem2 >= 2u * N ? 1u : 0u);
+  }
+  if (c.never) { lo = 0; hi = 255; return; }
+  uint64_t T = (uint64_t)__dsqrt_rd((double)c.W);
+  if (T > 0xffffffffull) T = 0xffffffffull;
+  while (T * T > c.W) --T;
+  while (T < 0xffffffffull && (T + 1) * (T + 1) <= c.W) ++T;
+  const uint64_t top = (uint64_t)S + T;
+  if (top >= 256ull * N) hi = 255;
+  else hi = (int)div_floor_u32((uint32_t)top, N, inv);         // top < 256 N <= 2^32
+  lo = (uint64_t)S > T ? (int)div_floor_u32((uint32_t)(S - T) + N - 1u, N, inv) : 0;   // S - T + N - 1 < 2^32: S <= 255 N, N <= 2^24
+  if (lo > hi) { lo = 1; hi = 0; }
+}
+
 __device__ __forceinline__ uint32_t warp_sum_u32(uint32_t v) {
 #pragma unroll
   for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);

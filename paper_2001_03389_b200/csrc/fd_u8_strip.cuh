@@ -46,6 +46,7 @@ struct FdStripParams {
   int64_t total_tiles;
   int off[4];                   // tensor path: x offset (bytes) of row class k inside its 16-byte aligned tensor
   int box_rows;                 // tensor path: rows per tensor copy (divides Rq / 4, <= 256)
+  uint32_t invC;                // ceil(2^32 / C) for C >= 2 (32-bit quotients of the bounds), else 0
 };
 
 // Tensor path.  Issuing one bulk copy per 128-byte row segment costs about ten warp instructions per copy
@@ -229,39 +230,58 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
     auto exchange = [&](bool first, int itn) {
       sync_all();                                                   // A: accumulators complete everywhere
       if (owner) {
-        uint32_t vs[8], vq[8];
-#pragma unroll
-        for (uint32_t q = 0; q < 8; ++q) {
-          vs[q] = 0; vq[q] = 0;
-          if (q < ncta) {
-            vs[q] = dsmem_ld_u32(dsmem_addr(&K->acc[buf][ocol], q));
-            vq[q] = dsmem_ld_u32(dsmem_addr(&K->acc[buf][kStripCols + ocol], q));
-          }
-        }
+        // The owners' chain sits between two barriers with everybody else waiting: keep it short.  Without a
+        // cluster everything is local shared memory; with one, all remote loads are issued before the first use.
         uint32_t s = 0, qq = 0;
+        if (ncta == 1) {
+          s = K->acc[buf][ocol];
+          qq = K->acc[buf][kStripCols + ocol];
+        } else {
+          uint32_t vs[8], vq[8];
 #pragma unroll
-        for (uint32_t q = 0; q < 8; ++q) { s += vs[q]; qq += vq[q]; }
+          for (uint32_t q = 0; q < 8; ++q) {
+            vs[q] = 0; vq[q] = 0;
+            if (q < ncta) {
+              vs[q] = dsmem_ld_u32(dsmem_addr(&K->acc[buf][ocol], q));
+              vq[q] = dsmem_ld_u32(dsmem_addr(&K->acc[buf][kStripCols + ocol], q));
+            }
+          }
+#pragma unroll
+          for (uint32_t q = 0; q < 8; ++q) { s += vs[q]; qq += vq[q]; }
+        }
         if (first) { colS = s; colQ = qq; } else { colS += s; colQ += qq; }   // deltas are modulo 2^32
         int lo = 0, hi = 255;
         uint32_t r = 0;
         if (ocol < tw) {
           const uint64_t V = (uint64_t)C * colQ - (uint64_t)colS * colS;
           const U8Cut cut = make_cut_u8((uint32_t)C, colS, V, P.p[itn]);
-          thread_bounds_u8_sqrt(cut, lo, hi);
-          r = rounded_mean_u8((uint32_t)C, colS);
+          if (P.invC) {
+            thread_bounds_u8_sqrt32(cut, P.invC, lo, hi, r);
+          } else {
+            thread_bounds_u8_sqrt(cut, lo, hi);
+            r = rounded_mean_u8((uint32_t)C, colS);
+          }
         }
         const int u = ocol & 3, slot = (u & 1) * 2 + (u >> 1);       // E.lo, O.lo, E.hi, O.hi
         const uint32_t neg = (0x10000u - ((uint32_t)lo << 8)) & 0xffffu;
         const uint32_t thr = lo > hi ? 0u : ((((uint32_t)(hi - lo)) << 8) | 0xffu);
         uint16_t* c16 = reinterpret_cast<uint16_t*>(&K->chk[ocol >> 2]);
+        if (ncta == 1) {
+          K->lo[ocol] = (uint8_t)lo;
+          K->hi[ocol] = (uint8_t)hi;
+          K->rr[ocol] = (uint8_t)r;
+          c16[slot] = (uint16_t)neg;
+          c16[4 + slot] = (uint16_t)thr;
+        } else {
 #pragma unroll
-        for (uint32_t q = 0; q < 8; ++q) {
-          if (q < ncta) {
-            dsmem_st_u8(dsmem_addr(&K->lo[ocol], q), (uint32_t)lo);
-            dsmem_st_u8(dsmem_addr(&K->hi[ocol], q), (uint32_t)hi);
-            dsmem_st_u8(dsmem_addr(&K->rr[ocol], q), r);
-            dsmem_st_u16(dsmem_addr(&c16[slot], q), neg);
-            dsmem_st_u16(dsmem_addr(&c16[4 + slot], q), thr);
+          for (uint32_t q = 0; q < 8; ++q) {
+            if (q < ncta) {
+              dsmem_st_u8(dsmem_addr(&K->lo[ocol], q), (uint32_t)lo);
+              dsmem_st_u8(dsmem_addr(&K->hi[ocol], q), (uint32_t)hi);
+              dsmem_st_u8(dsmem_addr(&K->rr[ocol], q), r);
+              dsmem_st_u16(dsmem_addr(&c16[slot], q), neg);
+              dsmem_st_u16(dsmem_addr(&c16[4 + slot], q), thr);
+            }
           }
         }
       }

@@ -424,6 +424,7 @@ int launch_fd_strip(const Call& c, const StripPlan& pl, int sms) {
   P.flags = c.flags;
   P.counts = c.counts;
   P.Rq = pl.rq;
+  P.invC = c.channels >= 2 ? (uint32_t)((((uint64_t)1 << 32) + (uint64_t)c.channels - 1) / (uint64_t)c.channels) : 0u;
   P.tiles_per_beam = (c.samples + rfim::kStripCols - 1) / rfim::kStripCols;
   P.total_tiles = (int64_t)P.tiles_per_beam * c.beams;
   rfim::FdStripMaps maps;

@@ -337,6 +337,7 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
           }
         }
       }
+      if (kTeam == 1 && !have_r) continue;                          // no group was touched (have_r is warp-uniform)
       team_sum3<kTeam>(cnt, sx, sxx, xchg, xsel, wt, lane, team);  // also orders the fixes before the next sweep
       cnt >>= 3;
       if (cnt) {
