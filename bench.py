@@ -40,7 +40,7 @@ FALLBACK_HBM_GBS = 6650.0        # /opt/skills/guides/B200_PROFILING.md, used on
 # launch bench.py times.  None until a capture exists.
 NCU_TRAFFIC = {
     "td_u8_staged": (9.253756e9 + 9.172766e9, 480, "profiles/r1b_td_details.txt"),
-    "fd_u8_strip1": (10.143028e9 + 9.176954e9, 480, "profiles/r1d_fd_details.txt"),
+    "fd_u8_strip1": (10.159767e9 + 9.180238e9, 480, "profiles/r1d_fd_details.txt"),
 }
 
 
