@@ -252,6 +252,12 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
       }
       s1 += s1b; s2 += s2b;
     }
+    // the team's next row travels HBM -> L2 while this one is iterated; its copy then comes from L2
+    if (tl == 0 && row + total_teams < P.rows) {
+      const uint8_t* gn = g + total_teams * P.stride;
+      const RowGeom gnx = row_geom(gn, S);
+      if (gnx.body > 0) bulk_prefetch_l2(gn + gnx.a0, (uint32_t)gnx.body);
+    }
     // totals fit 32 bits: the staged path is limited to S <= 65000 (S*255^2 < 2^32)
     team_sum3<kTeam>(s1, s2, s3, xchg, xsel, wt, lane, team);
     uint32_t xf = slot[h], xl = slot[h + S - 1];
