@@ -87,3 +87,12 @@ def test_binding_rejects_host_tensors():
         rfim.rfim_time_sigma_cut(x, [3.0])
     with pytest.raises(TypeError):
         binding._dtype_code(torch.zeros(1, dtype=torch.int32))
+
+
+def test_header_is_plain_c():
+    """include/rfim.h is the boundary: it must compile as C99 on its own (no C++ or CUDA types in the signatures)."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Werror", "-fsyntax-only", "-x", "c",
+                           os.path.join(root, "include", "rfim.h")])
