@@ -66,8 +66,7 @@ def test_config1_shape_fd(variant):
     x = synth.fill_host(cfg)
     name, counts = check(x, [3.0], variant=variant)
     assert name == ("fd_u8_strip1" if variant == TILE else "fd_u8_generic")
-    _, flags, _ = oracle.freq_sigma_cut(x, [3.0])
-    assert flags[0, 7].mean() > 0.9 and flags[0, 40].mean() > 0.9
+    # (the oracle-side pin P13 lives in tests/test_oracle_pins.py::test_p13_config1_behaviour)
 
 
 def test_config3_arts_like_all_beams():

@@ -17,6 +17,9 @@ its figures are images), so the oracle is pinned against what the definition
   P11 idempotence    a fixed point stays fixed
   P12 monotone       flagged(k2) subset of flagged(k1) for k1 < k2
   F*  FDSC           hand-computed binned column; bin-wise constant column
+  M*  median + bins  replacement = lower median of the flagged sample's own bin SNAPSHOT:
+                     rational brute force with sorted(), hand-computed columns, numpy (f32)
+  P13 behaviour      config 1: the 192 broadband-spike samples are cut by TDSC, the +60 channels by FDSC
 Every expected value in this file is derived by hand or by exact rational
 arithmetic in the test itself, never read back from the oracle.
 """
@@ -60,8 +63,10 @@ def brute_td_iteration(x, k):
     return [r if f else v for v, f in zip(x, flags)], flags
 
 
-def brute_fd_iteration(col, k, nb):
-    """One FDSC iteration on a column in exact rationals."""
+def brute_fd_iteration(col, k, nb, policy="mean"):
+    """One FDSC iteration on a column in exact rationals.  policy "median": a flagged
+    sample is replaced by the lower median (rank (nb-1)//2 of sorted()) of ITS bin's snapshot, i.e. of the
+    bin's values at the start of the iteration ("mean of its respective bin" + PAPER.md:110)."""
     C = len(col)
     kq = Fraction(int(round(k * K316)), K316)
     means = [Fraction(sum(col[b:b + nb]), nb) for b in range(0, C, nb)]
@@ -69,7 +74,10 @@ def brute_fd_iteration(col, k, nb):
     mu = sum(d) / C
     var = sum((v - mu) ** 2 for v in d) / C
     flags = [(v - mu) ** 2 > kq * kq * var for v in d]
-    rep = [(2 * sum(col[b:b + nb]) + nb) // (2 * nb) for b in range(0, C, nb)]
+    if policy == "median":
+        rep = [sorted(col[b:b + nb])[(nb - 1) // 2] for b in range(0, C, nb)]
+    else:
+        rep = [(2 * sum(col[b:b + nb]) + nb) // (2 * nb) for b in range(0, C, nb)]
     return [rep[c // nb] if flags[c] else col[c] for c in range(C)], flags
 
 
@@ -253,6 +261,94 @@ def test_p10_fd_u8_vs_exact_rationals(nbins, nb, data, ks):
     assert out[0, :, 0].tolist() == cur
     assert flags[0, :, 0].tolist() == [int(f) for f in anyflag]
     assert counts.tolist() == exp_counts
+
+
+@settings(max_examples=300, deadline=None)
+@given(st.integers(1, 6), st.sampled_from([1, 2, 3, 4, 5, 8]), st.data(),
+       st.lists(st.sampled_from([0.75, 1.0, 1.5, 2.0, 2.75]), min_size=1, max_size=3))
+def test_m1_fd_u8_median_with_bins_vs_exact_rationals(nbins, nb, data, ks):
+    """The median-with-bins branch of fdsc_iter_u8 (policy MEDIAN, bin_size < channels) against the brute
+    force: flags from exact rationals, replacement = sorted(bin snapshot)[(nb-1)//2].  A wrong bin offset, a
+    median taken after an earlier bin of the same iteration was modified, or an upper median fails here."""
+    C = nbins * nb
+    vals = data.draw(st.lists(st.integers(0, 255), min_size=C, max_size=C))
+    x = np.array(vals, dtype=np.uint8)
+    out, flags, counts = fd(x, ks, bin_size=nb, policy=oracle.MEDIAN)
+    cur = list(vals)
+    anyflag = [False] * C
+    exp_counts = []
+    for k in ks:
+        cur, fl = brute_fd_iteration(cur, k, nb, policy="median")
+        anyflag = [a or f for a, f in zip(anyflag, fl)]
+        exp_counts.append(sum(fl))
+    assert out[0, :, 0].tolist() == cur
+    assert flags[0, :, 0].tolist() == [int(f) for f in anyflag]
+    assert counts.tolist() == exp_counts
+
+
+@pytest.mark.parametrize("dtype", [np.uint8, np.float32])
+def test_m2_fd_median_with_bins_hand_computed(dtype):
+    """C = 8, bins of 4, column {1,2,3,40, 9,9,9,9}, k = 1.5, worked by hand.
+    Bin means 11.5 and 9; corrected {-10.5,-9.5,-8.5,28.5, 0,0,0,0}; their mean is 0 and
+    sigma'^2 = (110.25+90.25+72.25+812.25)/8 = 135.625, sigma' = 11.646, cut = 17.47: only the 40 is cut.
+    MEDIAN: sorted bin {1,2,3,40}, rank (4-1)//2 = 1 -> 2 (the LOWER median; the upper would be 3, the bin
+    mean 11.5 -> 12, the other bin's median 9, the whole column's lower median 9).
+    Second iteration (k = 1.5 again) on {1,2,3,2, 9,9,9,9}: bin means 2 and 9; corrected {-1,0,1,0,0,0,0,0};
+    sigma'^2 = 2/8, cut = 0.75: the 1 and the 3 are cut (dev 1) and replaced by the median of the snapshot
+    {1,2,3,2}: sorted {1,2,2,3}[1] = 2 -> {2,2,2,2, 9,9,9,9}; counts {1, 2}."""
+    col = np.array([1, 2, 3, 40, 9, 9, 9, 9], dtype=dtype)
+    out, flags, counts = fd(col, [1.5], bin_size=4, policy=oracle.MEDIAN)
+    assert out[0, :, 0].tolist() == [1, 2, 3, 2, 9, 9, 9, 9]
+    assert flags[0, :, 0].tolist() == [0, 0, 0, 1, 0, 0, 0, 0] and counts.tolist() == [1]
+    out, flags, counts = fd(col, [1.5, 1.5], bin_size=4, policy=oracle.MEDIAN)
+    assert out[0, :, 0].tolist() == [2, 2, 2, 2, 9, 9, 9, 9]
+    assert flags[0, :, 0].tolist() == [1, 0, 1, 1, 0, 0, 0, 0] and counts.tolist() == [1, 2]
+    # the mean policy on the same column: 40 -> round-half-up(11.5) = 12 (u8), 11.5 (f32)
+    out, _, _ = fd(col, [1.5], bin_size=4, policy=oracle.MEAN)
+    assert out[0, :, 0].tolist() == [1, 2, 3, 12 if dtype == np.uint8 else 11.5, 9, 9, 9, 9]
+    # flagged samples in BOTH bins of one iteration: each takes the median of its OWN bin's snapshot.
+    # {10,10,10,90, 50,50,52,120}, k = 1.5: bin means 30 and 68; corrected {-20,-20,-20,60,-18,-18,-16,52};
+    # sigma'^2 = (3*400+3600+324+324+256+2704)/8 = 1051, cut = 48.63: the 90 and the 120 are cut;
+    # medians: sorted {10,10,10,90}[1] = 10, sorted {50,50,52,120}[1] = 50.
+    col2 = np.array([10, 10, 10, 90, 50, 50, 52, 120], dtype=dtype)
+    out, flags, counts = fd(col2, [1.5], bin_size=4, policy=oracle.MEDIAN)
+    assert out[0, :, 0].tolist() == [10, 10, 10, 10, 50, 50, 52, 50]
+    assert flags[0, :, 0].tolist() == [0, 0, 0, 1, 0, 0, 0, 1] and counts.tolist() == [2]
+
+
+@pytest.mark.parametrize("policy", [oracle.MEAN, oracle.MEDIAN])
+@pytest.mark.parametrize("nb", [4, 8, 32])
+def test_m3_fd_f32_bins_vs_numpy(policy, nb):
+    """f32 FDSC with bins against numpy: bin means, np.std(ddof=0) of the mean-corrected values, np.sort per bin.
+    Samples closer than 1e-9 sigma to the cut are excluded (summation order)."""
+    rng = np.random.default_rng(11)
+    B, C, S = 2, 64, 40
+    x = rng.normal(0.0, 1.0, (B, C, S)).astype(np.float32)
+    x += np.repeat(rng.normal(0.0, 5.0, (B, C // nb, 1)), nb, axis=1).astype(np.float32)   # a bandpass shape
+    x[0, 13, :] += 7.0
+    x[1, 40, 5:25] -= 6.0
+    out, flags, counts = oracle.freq_sigma_cut(x, [2.75], policy=policy, bin_size=nb)
+    x64 = x.astype(np.float64).reshape(B, C // nb, nb, S)
+    m = x64.mean(axis=2, keepdims=True)
+    d = (x64 - m).reshape(B, C, S)
+    mu = d.mean(axis=1, keepdims=True)
+    sg = d.std(axis=1, ddof=0, keepdims=True)
+    dev = np.abs(d - mu)
+    safe = np.abs(dev - 2.75 * sg) > 1e-9 * sg
+    exp_flags = dev > 2.75 * sg
+    assert exp_flags.sum() > 40
+    assert np.array_equal(flags.astype(bool)[safe], exp_flags[safe])
+    if policy == oracle.MEAN:
+        rep = np.broadcast_to(m.astype(np.float32), x64.shape).reshape(B, C, S)
+    else:
+        srt = np.sort(x.reshape(B, C // nb, nb, S), axis=2)[:, :, (nb - 1) // 2, :]
+        rep = np.repeat(srt, nb, axis=1)
+    expect = np.where(flags.astype(bool), rep, x)
+    if policy == oracle.MEDIAN:
+        assert np.array_equal(out, expect)               # an element of the bin: exact
+    else:
+        np.testing.assert_allclose(out, expect, rtol=1e-6, atol=1e-6)
+    assert int(counts[0]) == int(flags.sum())
 
 
 def test_p10_f32_statistics_vs_numpy():
@@ -474,6 +570,28 @@ def test_fdsc_touches_only_its_column_and_td_only_its_row():
     assert np.array_equal(out_f, y)      # FDSC does not affect broadband signal
     out_t, flags_t, ct = oracle.time_sigma_cut(y, [3.0])
     assert ct[0] == 16 and np.all(out_t[0, :, 5] == 104)
+
+
+# ----------------------------------------------------------------------- P13
+def test_p13_config1_behaviour():
+    """SURVEY.md 8c P13 on the seeded config-1 input (BASELINE.json configs[0]): every one of the 3 x 64 = 192
+    broadband-spike samples (+80 = 8 sigma) is cut by TDSC at k = 3; the +60 channels 7 and 40 are NOT cleaned by
+    TDSC (a constant offset only moves the row mean) but are outliers across channels for FDSC."""
+    from paper_2001_03389_b200 import synth
+    cfg = synth.config(1)
+    x = synth.fill_host(cfg)
+    d = synth.Descriptor(cfg)
+    spikes = np.nonzero(d.imp_amp[0])[0]
+    assert len(spikes) == 3
+    out, flags, counts = oracle.time_sigma_cut(x, cfg["thresholds"])
+    assert flags[0][:, spikes].sum() == 64 * 3
+    assert abs(out[0, 7].astype(np.float64).mean() - 160) < 2 and abs(out[0, 40].astype(np.float64).mean() - 160) < 2
+    assert flags[0, 7].sum() <= 3 + 8 and flags[0, 40].sum() <= 3 + 8     # the spikes plus at most a few tail samples
+    _, fflags, _ = oracle.freq_sigma_cut(x, [3.0])
+    assert fflags[0, 7].mean() > 0.9 and fflags[0, 40].mean() > 0.9
+    others = np.ones(64, dtype=bool)
+    others[[7, 40]] = False
+    assert fflags[0, others].mean() < 0.02
 
 
 # --------------------------------------------------------------- ABI details
