@@ -13,9 +13,11 @@
  *       channels at a given time are grouped into bins, the bin mean is subtracted, each
  *       mean-corrected channel is compared to the mean-corrected statistics of all
  *       channels; an outlier's ORIGINAL value is replaced by the mean of its bin.
- *   Both take a list of thresholds: the production pipeline iterates ("three iterations
+ *   rfim_time_freq_sigma_cut   both, TDSC then FDSC on its result: the combination the paper
+ *       applies to every batch ("combined TDSC=3.25 sigma and FDSC=2.75 sigma").
+ *   All take a list of thresholds: the production pipeline iterates ("three iterations
  *   with 3.25 sigma"); iteration i sees the data cleaned by
- *   iteration i-1.  Both take a replacement strategy (mean | median).
+ *   iteration i-1.  All take a replacement strategy (mean | median).
  *
  * Exact definition (readings of the paper where it is silent: DESIGN.md "Readings"):
  *   population sigma; strict '>'; two-sided; statistics and replacement value are taken
@@ -26,16 +28,26 @@
  *
  * Layout: data[beam][channel][sample], sample fastest, rows `sample_stride` elements apart.
  *
- * Ownership / execution: every data pointer is a DEVICE pointer owned by the caller; the
- * library allocates no device memory for them and keeps no state between calls.  The
- * `thresholds` array is HOST memory, read before the call returns.  Work is enqueued on
- * `opts->stream` and the call returns without synchronising; no host read of device memory.
- * Scratch, when a kernel variant needs it, is taken from `opts->workspace`
- * (rfim_workspace_bytes says how much).
+ * Ownership / execution: every data pointer of the device entry points is a DEVICE pointer
+ * owned by the caller; the library allocates no device memory for them.  The `thresholds`
+ * arrays are HOST memory, read before the call returns.  Work is enqueued on `opts->stream`
+ * and the call returns without synchronising; no host read of device memory.  The library
+ * keeps no data between calls; it caches per-process launch attributes (shared-memory
+ * limits, occupancy) and the last tensor-map encodings, keyed on pointer and shape.
+ * `out` must be `data` itself (or NULL) or must not overlap it.
  *
- * Errors: return value only (no exceptions, errno or abort).  On any error nothing has
- * been enqueued.  There is no CPU fallback: a missing device or a failed launch is
- * RFIM_ERR_CUDA.
+ * Errors: return value only (no exceptions, errno or abort).  RFIM_ERR_INVALID and
+ * RFIM_ERR_UNSUPPORTED are decided before anything is enqueued.  RFIM_ERR_CUDA (a failed
+ * memset, copy or launch) leaves the outputs undefined: earlier operations of the same call
+ * may already be queued.  There is no CPU fallback: a missing device is RFIM_ERR_CUDA.
+ *
+ * Performance notes (DESIGN.md has the numbers): the tuned kernels are uint8 TDSC on whole rows
+ * of <= 65000 samples (mean or median), uint8 FDSC with mean replacement for channel counts of
+ * 512 / 1024 / 1536 / 2048 (one bin, or bins whose size is a multiple of 16 that divides
+ * channels / 4 ... see DESIGN.md) and, more slowly, any channel count that is a multiple of 4,
+ * and float32 TDSC.  Everything else the ABI accepts (uint8 windows, rows longer than 65000
+ * samples, FDSC with median replacement or odd bin sizes, float32 FDSC) runs in untuned
+ * one-thread-per-column / one-CTA-per-row kernels that go through L2 several times.
  */
 #ifndef RFIM_H
 #define RFIM_H
@@ -47,7 +59,7 @@
 extern "C" {
 #endif
 
-#define RFIM_VERSION 100 /* 0.1.0 */
+#define RFIM_VERSION 200 /* 0.2.0 */
 #define RFIM_MAX_THRESHOLDS 16
 
 typedef enum { RFIM_U8 = 0, RFIM_F32 = 1 } rfim_dtype;
@@ -56,9 +68,12 @@ typedef enum { RFIM_REPLACE_MEAN = 0, RFIM_REPLACE_MEDIAN = 1 } rfim_replace;
 enum {
   RFIM_OK = 0,
   RFIM_ERR_INVALID = -1,     /* bad argument (list below)                                  */
-  RFIM_ERR_UNSUPPORTED = -2, /* valid request that no kernel implements yet                */
+  RFIM_ERR_UNSUPPORTED = -2, /* valid request that no kernel (of the forced variant) runs  */
   RFIM_ERR_CUDA = -3         /* CUDA runtime error (text: rfim_last_cuda_error)            */
 };
+
+/* rfim_workspace_bytes `op` */
+enum { RFIM_OP_TIME = 0, RFIM_OP_FREQ = 1, RFIM_OP_TIME_FREQ = 2, RFIM_OP_HOST = 3 };
 
 typedef struct {
   int64_t   sample_stride; /* elements between consecutive (beam,channel) rows; 0 = samples (dense) */
@@ -67,16 +82,17 @@ typedef struct {
   void*     out;           /* device; NULL = in place; else same shape/stride as data (may == data) */
   uint8_t*  flags;         /* device, optional dense [B][C][S]; 1 = replaced in ANY iteration, else 0 */
   uint64_t* counts;        /* device, optional [n_thresholds]; samples replaced in iteration i
-                              (overwritten, not accumulated; a sample can be counted twice)        */
+                              (overwritten, not accumulated; a sample can be counted twice);
+                              rfim_time_freq_sigma_cut: [n_time + n_freq], time iterations first    */
   void*     stream;        /* cudaStream_t; NULL = legacy default stream                            */
   void*     workspace;     /* device scratch of >= rfim_workspace_bytes(...) bytes, or NULL        */
   int32_t   variant;       /* 0 = auto.  Non-zero selects a kernel variant (testing / tuning):
-                              1 = generic (any alignment, any row length), 2 = fast path (staged TDSC /
-                              strip FDSC), 3 / 4 = staged TDSC with one / two warps per row,
-                              5 / 6 / 7 / 8 = wide-tile cluster FDSC with 1 / 2 / 4 / 8 CTAs per tile, 11 / 12 =
-                              the same with 4 / 8 CTAs and one thread per word column, 13 = strip FDSC with
-                              per-row bulk copies, 14 = strip FDSC, never the whole tile in one CTA.
-                              A variant that cannot run the request returns RFIM_ERR_UNSUPPORTED.  */
+                              1 = generic correctness kernels, 2 = a tuned kernel or RFIM_ERR_UNSUPPORTED;
+                              TDSC only: 3 / 4 = staged kernel with one / two warps per row;
+                              FDSC only: 13 = strip kernel with per-row bulk copies, 14 = strip kernel in
+                              clusters (never the whole tile in one CTA), 15 = strip kernel, 16 = streaming
+                              kernel.  A variant that cannot run the request, or belongs to the other
+                              operation, returns RFIM_ERR_UNSUPPORTED.                              */
   int32_t   reserved;      /* must be 0                                                            */
 } rfim_opts;               /* opts == NULL means all zeros                                          */
 
@@ -89,8 +105,8 @@ typedef struct {
  *                 (the last window of a row may be shorter); 0 = the whole row (the paper's batch)
  * RFIM_ERR_INVALID: NULL data; a dimension <= 0; n_thresholds outside [0,16]; NULL thresholds with
  *   n > 0; a threshold that is NaN, <= 0 or >= 256; sample_stride in (0, samples); window < 0;
- *   bin_size < 0; unknown enum; RFIM_U8 with samples > 2^24; reserved != 0; flags/counts/out
- *   misaligned for their type.
+ *   bin_size < 0; unknown enum or variant; RFIM_U8 with samples > 2^24; reserved != 0; flags/counts/out
+ *   misaligned for their type; out overlapping data without being data.
  * n_thresholds == 0 is a valid no-op (copies data to out when out-of-place).
  */
 int rfim_time_sigma_cut(void* data, int beams, int channels, int samples, rfim_dtype dtype,
@@ -102,6 +118,7 @@ int rfim_time_sigma_cut(void* data, int beams, int channels, int samples, rfim_d
  *   As above, statistics across the `channels` axis for every (beam, sample).
  *   opts->bin_size  channels per bin for step 1 (bin-mean correction); must divide channels;
  *                   0 = one bin of all channels (then FDSC is TDSC along the channel axis).
+ * In place, a sample that is not replaced is not rewritten.
  * Additional RFIM_ERR_INVALID: bin_size not dividing channels; RFIM_U8 with channels > 2^24 or
  *   1 < bin_size < channels with bin_size > 65536.
  */
@@ -110,19 +127,34 @@ int rfim_freq_sigma_cut(void* data, int beams, int channels, int samples, rfim_d
                         const rfim_opts* opts);
 
 /*
+ * TDSC followed by FDSC on its result -- PAPER.md:118,144.  Equivalent to rfim_time_sigma_cut(data -> out)
+ * followed by rfim_freq_sigma_cut(out, in place), on the same stream: TDSC reads `data` and writes `out` (or
+ * works in place), FDSC then cleans that result in place.  opts->window applies to TDSC, opts->bin_size to
+ * FDSC; flags = replaced by either; counts = [n_time + n_freq].  Either list may be empty.
+ */
+int rfim_time_freq_sigma_cut(void* data, int beams, int channels, int samples, rfim_dtype dtype,
+                             const double* time_thresholds, int n_time,
+                             const double* freq_thresholds, int n_freq,
+                             rfim_replace policy, const rfim_opts* opts);
+
+/*
  * Host-buffer convenience (end-to-end path): `data` and `out` are HOST pointers (pinned memory
- * gives full PCIe rate; pageable works).  Beams are streamed through device staging buffers the
- * call allocates and frees itself: H2D copy, rfim_time_sigma_cut (if n_time > 0), then
- * rfim_freq_sigma_cut (if n_freq > 0) on the device, D2H copy, overlapped across beams.  Synchronous:
- * returns when `out` (or `data`, if out is NULL) holds the result.  opts->out / flags / counts /
- * stream / workspace must be NULL here; sample_stride, window, bin_size apply.
+ * gives full PCIe rate; pageable works).  Beams are streamed in chunks through three device staging
+ * buffers: H2D copy, rfim_time_freq_sigma_cut on the chunk, D2H copy, overlapped across chunks on three
+ * internal streams.  The staging buffers are taken from opts->workspace (device memory of at least
+ * rfim_workspace_bytes(RFIM_OP_HOST, ...) bytes); with workspace == NULL the call allocates and frees
+ * them itself (slower: a cudaMalloc / cudaFree pair per call).  Synchronous: returns when `out` (or
+ * `data`, if out is NULL) holds the result.  opts->out / flags / counts / stream must be NULL here;
+ * sample_stride, window, bin_size, workspace apply.  Only the operations that run (n_time > 0, n_freq > 0)
+ * are validated.  On RFIM_ERR_CUDA `out` may be partly written.
  */
 int rfim_sigma_cut_host(void* data, void* out, int beams, int channels, int samples, rfim_dtype dtype,
                         const double* time_thresholds, int n_time,
                         const double* freq_thresholds, int n_freq,
                         rfim_replace policy, const rfim_opts* opts);
 
-/* Bytes of device scratch the given call needs in opts->workspace (0 = none). `op`: 0 time, 1 freq. */
+/* Bytes of device scratch the given call uses from opts->workspace (0 = none).  `op`: RFIM_OP_*.  The device
+ * entry points need none today; RFIM_OP_HOST returns the size of the three staging buffers. */
 size_t rfim_workspace_bytes(int op, int beams, int channels, int samples, rfim_dtype dtype,
                             int n_thresholds, rfim_replace policy, const rfim_opts* opts);
 

@@ -18,9 +18,11 @@ MEAN, MEDIAN = 0, 1
 OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_CUDA = 0, -1, -2, -3
 VARIANT_AUTO, VARIANT_GENERIC, VARIANT_STAGED = 0, 1, 2
 VARIANT_STAGED_1W, VARIANT_STAGED_2W = 3, 4
-VARIANT_FD_CL1, VARIANT_FD_CL2, VARIANT_FD_CL4, VARIANT_FD_CL8 = 5, 6, 7, 8
+VARIANT_FD_STRIP_BULK, VARIANT_FD_STRIP_CLUSTER, VARIANT_FD_STRIP, VARIANT_FD_STREAM = 13, 14, 15, 16
+OP_TIME, OP_FREQ, OP_TIME_FREQ, OP_HOST = 0, 1, 2, 3
 
-EXPORTS = ("rfim_time_sigma_cut", "rfim_freq_sigma_cut", "rfim_sigma_cut_host", "rfim_workspace_bytes",
+EXPORTS = ("rfim_time_sigma_cut", "rfim_freq_sigma_cut", "rfim_time_freq_sigma_cut", "rfim_sigma_cut_host",
+           "rfim_workspace_bytes",
            "rfim_launch_count", "rfim_last_variant", "rfim_status_string", "rfim_last_cuda_error",
            "rfim_version")
 
@@ -67,6 +69,10 @@ def lib() -> ctypes.CDLL:
         for name in ("rfim_time_sigma_cut", "rfim_freq_sigma_cut"):
             getattr(_lib, name).argtypes = sig
             getattr(_lib, name).restype = ctypes.c_int
+        _lib.rfim_time_freq_sigma_cut.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
+                                                  ctypes.c_int, dp, ctypes.c_int, dp, ctypes.c_int, ctypes.c_int,
+                                                  ctypes.POINTER(RfimOpts)]
+        _lib.rfim_time_freq_sigma_cut.restype = ctypes.c_int
         _lib.rfim_sigma_cut_host.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int, ctypes.c_int,
                                              ctypes.c_int, ctypes.c_int, dp, ctypes.c_int, dp, ctypes.c_int,
                                              ctypes.c_int, ctypes.POINTER(RfimOpts)]
@@ -169,10 +175,50 @@ def rfim_freq_sigma_cut(data: torch.Tensor, thresholds: Sequence[float], policy=
                  workspace)
 
 
+def rfim_time_freq_sigma_cut(data: torch.Tensor, time_thresholds: Sequence[float], freq_thresholds: Sequence[float],
+                             policy=MEAN, *, out: Optional[torch.Tensor] = None, window: int = 0, bin_size: int = 0,
+                             flags: Optional[torch.Tensor] = None, counts: Optional[torch.Tensor] = None,
+                             stream=None, variant: int = VARIANT_AUTO) -> torch.Tensor:
+    """TDSC then FDSC on its result.  Asynchronous on `stream`; TDSC writes `out` (or works in
+    place), FDSC cleans that result in place.  counts: int64 [len(time) + len(freq)]."""
+    if not data.is_cuda:
+        raise ValueError("librfim: data must be a CUDA tensor (device pointer ABI; no CPU fallback)")
+    b, c, s, pitch = _layout(data)
+    if out is not None:
+        if out.shape != data.shape or out.dtype != data.dtype or _layout(out)[3] != pitch or not out.is_cuda:
+            raise ValueError("librfim: out must match data in shape, dtype and pitch")
+    if flags is not None and (flags.dtype != torch.uint8 or not flags.is_contiguous() or flags.numel() != b * c * s):
+        raise ValueError("librfim: flags must be a dense uint8 [B][C][S] tensor")
+    tt, nt = _doubles(time_thresholds)
+    ft, nf = _doubles(freq_thresholds)
+    if counts is not None and (counts.dtype != torch.int64 or counts.numel() < nt + nf):
+        raise ValueError("librfim: counts must be int64 with n_time + n_freq entries")
+    if stream is None:
+        stream = torch.cuda.current_stream(data.device)
+    o = RfimOpts(pitch if pitch != s else 0, int(window), int(bin_size),
+                 out.data_ptr() if out is not None else None,
+                 flags.data_ptr() if flags is not None else None,
+                 counts.data_ptr() if counts is not None else None,
+                 stream.cuda_stream, None, int(variant), 0)
+    with torch.cuda.device(data.device):
+        st = lib().rfim_time_freq_sigma_cut(data.data_ptr(), b, c, s, _dtype_code(data), tt, nt, ft, nf,
+                                            _policy_code(policy), ctypes.byref(o))
+    _check(st)
+    return out if out is not None else data
+
+
+def rfim_workspace_bytes(op: int, beams: int, channels: int, samples: int, dtype=U8, n_thresholds: int = 0,
+                         policy=MEAN, sample_stride: int = 0) -> int:
+    o = RfimOpts(int(sample_stride), 0, 0, None, None, None, None, None, 0, 0)
+    return int(lib().rfim_workspace_bytes(int(op), beams, channels, samples, int(dtype), n_thresholds,
+                                          _policy_code(policy), ctypes.byref(o)))
+
+
 def rfim_sigma_cut_host(data: torch.Tensor, time_thresholds: Sequence[float], freq_thresholds: Sequence[float],
                         policy=MEAN, *, out: Optional[torch.Tensor] = None, window: int = 0,
-                        bin_size: int = 0) -> torch.Tensor:
-    """End-to-end path on HOST tensors (pinned memory recommended): H2D, TDSC, FDSC, D2H, streamed by beam."""
+                        bin_size: int = 0, workspace: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """End-to-end path on HOST tensors (pinned memory recommended): H2D, TDSC, FDSC, D2H, streamed by beam.
+    `workspace`: device tensor of >= rfim_workspace_bytes(OP_HOST, ...) bytes for the staging buffers."""
     if data.is_cuda:
         raise ValueError("rfim_sigma_cut_host takes host tensors")
     b, c, s, pitch = _layout(data)
@@ -180,7 +226,12 @@ def rfim_sigma_cut_host(data: torch.Tensor, time_thresholds: Sequence[float], fr
         raise ValueError("librfim: out must match data in shape, dtype and pitch")
     tt, nt = _doubles(time_thresholds)
     ft, nf = _doubles(freq_thresholds)
-    o = RfimOpts(pitch if pitch != s else 0, int(window), int(bin_size), None, None, None, None, None, 0, 0)
+    if workspace is not None:
+        need = rfim_workspace_bytes(OP_HOST, b, c, s, _dtype_code(data), sample_stride=pitch if pitch != s else 0)
+        if not workspace.is_cuda or workspace.numel() * workspace.element_size() < need:
+            raise ValueError(f"librfim: workspace must be a CUDA tensor of at least {need} bytes")
+    o = RfimOpts(pitch if pitch != s else 0, int(window), int(bin_size), None, None, None, None,
+                 workspace.data_ptr() if workspace is not None else None, 0, 0)
     st = lib().rfim_sigma_cut_host(data.data_ptr(), out.data_ptr() if out is not None else None, b, c, s,
                                    _dtype_code(data), tt, nt, ft, nf, _policy_code(policy), ctypes.byref(o))
     _check(st)

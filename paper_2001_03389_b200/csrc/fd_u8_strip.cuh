@@ -1,24 +1,28 @@
 // fd_u8_strip.cuh -- frequency-domain sigma cut (FDSC, Fig. 3) for uint8 dynamic spectra,
 // one bin of all channels: the strip kernel.
 //
-// A tile is ALL channels x 128 consecutive samples of one beam (a strip).  A thread-block cluster of NC CTAs
-// (NC = 2 for 1536 channels) owns one tile at a time; CTA q holds channels [q*Rq, (q+1)*Rq) in shared memory
-// as rows of 144 bytes (110 KB for 768 rows: two CTAs per SM, so one tile's copies overlap the other's
-// arithmetic).  Why strips and small clusters: every exchange of column statistics is a cluster-wide barrier,
-// and a barrier over many CTAs waits for the slowest of them four times per tile; with whole columns in two
-// CTAs the exchange is 128 columns between two neighbours.
-//   F1: one 1-D TMA bulk copy per row segment (the 16-byte aligned superset of its 128 bytes: rows of a dense
-//       [C][S] beam are only 4-byte aligned), all completing on one mbarrier.
-//   F2: lane = word column (32 lanes x 4 samples = the strip), warp w owns rows w, w+16, ...: a warp reads 32
-//       consecutive words of one row (no bank conflicts).  4x4 byte transposes (PRMT) turn four rows into
-//       words that each hold ONE column, so IDP.4A gives exact column sums and sums of squares; the sixteen
-//       warps meet in shared-memory accumulators (RED.ADD).
-//   F3: column c is owned by one thread of one CTA, which adds up the accumulators of all CTAs (DSMEM loads,
-//       issued together), keeps (S, Q) in registers across iterations, computes the exact kept interval
-//       [lo, hi] in closed form (integer square root) and r, and pushes them to every CTA (DSMEM stores).
+// The general fast kernel: any channel count that is a multiple of 4 (up to ~12 K channels through clusters of
+// CTAs).  The streaming kernel of fd_u8_stream.cuh is preferred for the channel counts it takes.
+//
+// A tile is ALL channels x 128 consecutive samples of one beam (a strip), resident in shared memory as rows of
+// 144 bytes.  Whenever it fits (<= 1576 channels) ONE CTA of 32 warps holds the whole tile (216 KB, one CTA per
+// SM, only __syncthreads); otherwise the channels are split over the smallest thread-block cluster that fits,
+// CTA q holding channels [q*Rq, (q+1)*Rq), and column statistics / bounds cross the cluster through DSMEM.
+//   F1: TMA tensor copies, one box per warp (or per alignment class): the rows of one 16-byte alignment class
+//       (row mod 4) form a 2-D tensor even on the dense 4-byte aligned pitch; a box is the 144-byte aligned
+//       superset of the 128 columns.  Fallback (channels % 4 != 0, variant 13): one 1-D bulk copy per row.
+//   F2: lane = word column (32 lanes x 4 samples = the strip); a warp reads 32 consecutive words of one row (no
+//       bank conflicts).  4x4 byte transposes (PRMT) turn four rows into words that each hold ONE column, so
+//       IDP.4A gives exact column sums and sums of squares; the warps meet in shared-memory accumulators (RED.ADD).
+//   F3: column c is owned by one thread of one CTA, which adds up the accumulators of all CTAs, keeps (S, Q) in
+//       registers across iterations, computes the exact kept interval [lo, hi] in closed form (integer square
+//       root) and r, and publishes them to every CTA.
 //   F4: packed range check per four rows (VIADDMNMX.U16x2) records which steps hold an outlier; the exact
 //       repair runs afterwards over the recorded steps only; column deltas go to the accumulators.
-//   F5: next threshold from the updated (S, Q).  F6: bulk store per row segment + ragged ends.
+//   F5: next threshold from the updated (S, Q).  F6: the last sweep writes the rows it finds clean straight from
+//       its registers, the repair writes the others: one coalesced 32-bit store per lane and row (the 144-byte
+//       superset cannot be stored back by TMA: its margins belong to the neighbouring tiles, a tensor box must
+//       start on a 16-byte boundary and TMA stores clip at 16-byte granularity).
 #pragma once
 
 #include <cuda.h>   // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
@@ -61,19 +65,12 @@ struct FdStripParams {
 // per lane.
 struct FdStripMaps {
   CUtensorMap src[4];
-  CUtensorMap dst[4];
 };
 __device__ __forceinline__ void tma_load_2d(void* smem_dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
   asm volatile(
       "cp.async.bulk.tensor.2d.shared::cluster.global.tile.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
       ::"r"(smem_addr(smem_dst)), "l"(reinterpret_cast<uint64_t>(map)), "r"(x), "r"(y), "r"(smem_addr(bar))
       : "memory");
-}
-__device__ __forceinline__ void tma_store_2d(const CUtensorMap* map, int x, int y, const void* smem_src) {
-  asm volatile("cp.async.bulk.tensor.2d.global.shared::cta.tile.bulk_group [%0, {%1, %2}], [%3];" ::"l"(
-                   reinterpret_cast<uint64_t>(map)),
-               "r"(x), "r"(y), "r"(smem_addr(smem_src))
-               : "memory");
 }
 // bring a box into L2 only (no shared-memory destination, no completion to wait for)
 __device__ __forceinline__ void tma_prefetch_l2_2d(const CUtensorMap* map, int x, int y) {

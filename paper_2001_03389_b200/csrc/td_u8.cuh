@@ -13,7 +13,10 @@
 //       the groups it found by itself (exact per-byte masks, replace, S and Q deltas, summary
 //       refresh), so there is no queue, atomic or barrier.  T5: next threshold, on chip, from the
 //       updated S, Q and summaries.  T6: one TMA bulk store.  HBM sees one read and one write per
-//       sample.
+//       sample.  Median replacement (kMedian): the replacement value of an iteration is the lower
+//       median of the snapshot, found -- only in rows where the iteration cuts something, at the first hit and
+//       therefore before any replacement -- by counting passes over the staged row (bytes <= v, packed compares
+//       + IDP.4A) that start at the rounded mean and bracket, then bisect, the rank.
 //   td_u8_generic_kernel  any alignment / stride / row length / window, mean or median: one CTA per
 //       row, byte loads, iterations through global memory (L1/L2).  Correctness path, not tuned.
 #pragma once
@@ -126,6 +129,51 @@ __device__ __forceinline__ void warp_bounds_u8_fast(const U8Cut& c, float k, uin
   if (!ok) warp_bounds_u8(c, lane, lo, hi);
 }
 
+// T2m: number of bytes <= v among the J 16-byte groups of a staged row (padding included), by one warp
+__device__ __forceinline__ uint32_t warp_count_le(const uint4* s4, int J, uint32_t v, int lane) {
+  const uint32_t cab2 = (0x7fffu - v) * 0x00010001u;              // bytes_above(w, cab2): bytes > v
+  uint32_t n = 0;
+  for (int gi = lane; gi < J; gi += 32) {
+    const uint4 w = s4[gi];
+    n = __dp4a(~bytes_above(w.x, cab2) & 0x01010101u, 0x01010101u, n);
+    n = __dp4a(~bytes_above(w.y, cab2) & 0x01010101u, 0x01010101u, n);
+    n = __dp4a(~bytes_above(w.z, cab2) & 0x01010101u, 0x01010101u, n);
+    n = __dp4a(~bytes_above(w.w, cab2) & 0x01010101u, 0x01010101u, n);
+  }
+  return __reduce_add_sync(FULL, n);
+}
+// Lower median (rank (S - 1) / 2 of the ascending snapshot) of the row staged at slot[h .. h + S): the smallest v
+// with #{x <= v} > rank.  hpad / epad copies of xf / xl pad the first / last group and are taken out of every
+// count.  The search starts at `guess` (the rounded mean), gallops to a bracket and bisects: two or three
+// counting passes for noise-like rows, at most about twelve.
+__device__ __forceinline__ uint32_t warp_lower_median_u8(const uint4* s4, int J, int S, int hpad, int epad, uint32_t xf,
+                                                         uint32_t xl, uint32_t guess, int lane) {
+  const uint32_t rank = (uint32_t)(S - 1) >> 1;
+  auto above = [&](uint32_t v) {                                  // #{x <= v} > rank ?
+    uint32_t n = warp_count_le(s4, J, v, lane);
+    n -= (xf <= v ? (uint32_t)hpad : 0u) + (xl <= v ? (uint32_t)epad : 0u);
+    return n > rank;
+  };
+  int lo, hi;                                                     // the median lies in [lo, hi]
+  int g = (int)min(guess, 255u);
+  if (above((uint32_t)g)) {
+    hi = g; lo = 0;
+    for (int step = 1; hi - step >= 0; step <<= 1) {
+      if (above((uint32_t)(hi - step))) { hi -= step; } else { lo = hi - step + 1; break; }
+    }
+  } else {
+    lo = g + 1; hi = 255;
+    for (int step = 1; lo + step - 1 <= 255; step <<= 1) {
+      if (above((uint32_t)(lo + step - 1))) { hi = lo + step - 1; break; } else { lo += step; }
+    }
+  }
+  while (lo < hi) {
+    const int mid = (lo + hi) >> 1;
+    if (above((uint32_t)mid)) hi = mid; else lo = mid + 1;
+  }
+  return (uint32_t)lo;
+}
+
 // A team of kTeam warps (1 or 2) owns one shared-memory slot and one row at a time; sixteen teams
 // per SM keep sixteen rows in flight, which is what covers the HBM latency (measured: fewer teams
 // with two slots each are slower).  kTeam = 2 doubles the warps per SM for the same shared memory.
@@ -176,8 +224,9 @@ __device__ __forceinline__ RowGeom row_geom(const uint8_t* g, int S) {
   return r;
 }
 
-template <int kTeam, bool kFlags>
+template <int kTeam, bool kFlags, bool kMedian>
 __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8Params P) {
+  static_assert(!(kMedian && kTeam != 1), "the snapshot median is taken by the one warp that owns the row");
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr int TL = 32 * kTeam;                                  // threads per team
   const int lane = threadIdx.x & 31;
@@ -314,7 +363,9 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
         const bool hit = ah != HI2 || al != LO2;
         if (!__any_sync(FULL, hit)) continue;
         if (!have_r) {
+          // first hit of this iteration: nothing has been replaced yet, the slot still holds the snapshot
           r = rounded_mean_u8((uint32_t)S, Ssum);
+          if (kMedian) r = warp_lower_median_u8(s4, J, S, h, geo.pe, xf, xl, r, lane);
           r4 = r * 0x01010101u;
           have_r = true;
         }

@@ -14,7 +14,17 @@ pytestmark = pytest.mark.gpu
 
 DEV = "cuda:0"
 TILE, GENERIC = rfim.VARIANT_STAGED, rfim.VARIANT_GENERIC
-CL1, CL2, CL4, CL8 = 5, 6, 7, 8          # rfim_opts.variant: force the cluster size of the FDSC kernel
+STRIP, STRIP_BULK, STRIP_CLUSTER, STREAM = (rfim.VARIANT_FD_STRIP, rfim.VARIANT_FD_STRIP_BULK,
+                                            rfim.VARIANT_FD_STRIP_CLUSTER, rfim.VARIANT_FD_STREAM)
+
+
+def fast_name(C, S, inplace=False):
+    """The tuned kernel auto mode picks for a dense [.][C][S] uint8 request with mean replacement and one bin."""
+    if S % 4 != 0:
+        return "fd_u8_generic"
+    if C in (512, 1024, 1536, 2048):
+        return "fd_u8_stream" if inplace else "fd_u8_stream_copy"
+    return "fd_u8_strip"
 
 
 def run_gpu(x_np, ks, variant=rfim.VARIANT_AUTO, inplace=False, pitch=None, want_flags=True):
@@ -77,8 +87,12 @@ def test_config3_arts_like_all_beams():
     synth.fill_device(cfg, x)
     x_np = x.cpu().numpy()
     name, counts = check(x_np, cfg["thresholds"], inplace=True)
-    assert name == "fd_u8_strip1"
+    assert name == "fd_u8_stream"
     assert all(int(c) > 0 for c in counts)
+    name, _ = check(x_np[:3], cfg["thresholds"])                      # out of place: copy + repair
+    assert name == "fd_u8_stream_copy"
+    name, _ = check(x_np[:2], cfg["thresholds"], inplace=True, variant=STRIP)
+    assert name == "fd_u8_strip1"
     check(x_np[:1], cfg["thresholds"], variant=GENERIC)
 
 
@@ -109,8 +123,7 @@ def test_shapes(C, S, variant):
         x[1, C - 1, S - 1] = 0
         x[0, :, 0] = 77                                                                          # constant column
     name, _ = check(x, [4.0, 3.0], variant=variant)
-    tiled = variant != GENERIC and S % 4 == 0
-    assert name.startswith("fd_u8_strip") == tiled, name
+    assert name.startswith("fd_u8_generic" if variant == GENERIC else fast_name(C, S)), name
     check(x, [3.25, 3.25, 3.25], variant=variant, inplace=True)
 
 
@@ -131,7 +144,7 @@ def test_misaligned_out():
     xd = torch.from_numpy(x).to(DEV)
     ref, _, _ = oracle.freq_sigma_cut(x, [3.0])
     for shift, want in ((4, "fd_u8_generic"), (1, "fd_u8_generic"), (16, "fd_u8_strip1")):
-        obuf = torch.zeros(16 * 1000 + 32, dtype=torch.uint8, device=DEV)
+        obuf = torch.zeros(16 * 1000 + 64, dtype=torch.uint8, device=DEV)
         out = obuf[shift:shift + 16000].view(1, 16, 1000)
         rfim.rfim_freq_sigma_cut(xd, [3.0], out=out)
         torch.cuda.synchronize()
@@ -142,6 +155,11 @@ def test_misaligned_out():
     with pytest.raises(rfim.RfimError) as e:
         rfim.rfim_freq_sigma_cut(xd, [3.0], out=out, variant=TILE)
     assert e.value.status == -2
+    # out overlapping data without being data is refused (include/rfim.h)
+    big = torch.zeros(2 * 16000, dtype=torch.uint8, device=DEV)
+    with pytest.raises(rfim.RfimError) as e:
+        rfim.rfim_freq_sigma_cut(big[:16000].view(1, 16, 1000), [3.0], out=big[8000:24000].view(1, 16, 1000))
+    assert e.value.status == -1
 
 
 def test_unaligned_base_pointer_tile_path():
@@ -209,8 +227,7 @@ def test_many_tiles_grid_wraps():
     assert name == "fd_u8_strip1"
     name, _ = check(np.ascontiguousarray(x[:, :, :2096]), [4.0, 3.0])
     assert name == "fd_u8_strip1"
-    for v in (CL2, CL4, CL8):
-        check(x[:13], [4.0, 3.0], variant=v)
+    check(x[:13], [4.0, 3.0], variant=STRIP_CLUSTER)
 
 
 def test_no_flags_no_counts_other_stream():
@@ -241,38 +258,6 @@ def test_unsupported_requests_fail_loudly():
     assert e.value.status == -2
 
 
-# ------------------------------------------------------------------------ forced cluster sizes
-@pytest.mark.parametrize("variant,name", [(CL1, "fd_u8_cluster1"), (CL2, "fd_u8_cluster2"), (CL4, "fd_u8_cluster4"),
-                                          (CL8, "fd_u8_cluster8")])
-@pytest.mark.parametrize("C,S", [(3, 64), (8, 100), (37, 1000), (200, 520), (1000, 2100), (1536, 700)])
-def test_cluster_sizes(variant, name, C, S):
-    """Channels split over 1, 2, 4, 8 CTAs: uneven splits, CTAs without any channel (C < cluster size), several
-    tiles per beam with a ragged last one, partial sums and column deltas exchanged through DSMEM."""
-    x = noisy((3, C, S), seed=C + S)
-    if C > 1020 * (1 << (variant - CL1)):
-        # more than 1020 channels per CTA: the packed per-thread delta counters would overflow, so the
-        # library refuses the forced variant (auto picks a larger cluster)
-        with pytest.raises(rfim.RfimError) as e:
-            run_gpu(x, [4.0], variant=variant)
-        assert e.value.status == -2
-        return
-    x[0, C // 2, :] = np.minimum(x[0, C // 2, :].astype(int) + 90, 255).astype(np.uint8)
-    x[1, :, S // 3] = 3
-    x[2, C - 1, ::3] = 255
-    got, _ = check(x, [4.0, 3.0, 3.0], variant=variant)
-    assert got == name
-    check(x, [3.25, 3.25], variant=variant, inplace=True)
-
-
-def test_cluster_pitch_and_phase():
-    """Padded pitches with every 16-byte phase pattern, through the 8-CTA cluster."""
-    for pitch in (1008, 1004, 1012, 1024):
-        x = noisy((2, 100, 1000), seed=pitch)
-        x[:, 9, :] = 200
-        check(x, [4.0, 3.0], pitch=pitch, variant=CL8)
-        check(x, [4.0, 3.0], pitch=pitch, variant=CL4, inplace=True)
-
-
 # ------------------------------------------------------------------------ strip kernel: cluster sizes by channel count
 @pytest.mark.parametrize("C,name", [(700, "fd_u8_strip1_bulk"), (768, "fd_u8_strip1"), (1537, "fd_u8_strip1_bulk"), (3001, "fd_u8_strip4_bulk"),
                                     (6100, "fd_u8_strip8_bulk"), (1536, "fd_u8_strip1"), (3072, "fd_u8_strip4"),
@@ -285,10 +270,12 @@ def test_strip_cluster_sizes(C, name):
     x[0, ::97, :] = 250
     x[1, C // 2:C // 2 + 40, 17:60] = 0
     x[1, :, 299] = 7
-    got, _ = check(x, [4.0, 3.0])
+    got, _ = check(x, [4.0, 3.0], variant=STRIP)       # (auto prefers the streaming kernel for 1024 / 1536 channels)
     assert got == name
-    check(x, [0.5, 3.0, 3.0], inplace=True)
-    got, _ = check(x, [4.0, 3.0], variant=13)          # the same kernel with per-row bulk copies
+    got, _ = check(x, [4.0, 3.0])
+    assert got == ("fd_u8_stream_copy" if C in (1024, 1536) else name)
+    check(x, [0.5, 3.0, 3.0], inplace=True, variant=STRIP)
+    got, _ = check(x, [4.0, 3.0], variant=STRIP_BULK)  # the same kernel with per-row bulk copies
     assert got == name.replace("_bulk", "") + "_bulk"
-    got, _ = check(x, [4.0, 3.0], variant=14)          # never the whole tile in one CTA: clusters, two CTAs per SM
+    got, _ = check(x, [4.0, 3.0], variant=STRIP_CLUSTER)   # never the whole tile in one CTA: clusters, two CTAs per SM
     assert got.startswith("fd_u8_strip2" if C in (1536, 1537, 1028, 1024, 1280, 1152) else name.replace("_bulk", ""))

