@@ -65,6 +65,7 @@ struct FdStreamParams {
   uint32_t invC;                                   // ceil(2^32 / C)
   int nb, nbins;                                   // binned: channels per bin (multiple of 16), bins
   uint32_t inv_nb, inv_2nb;                        // ceil(2^32 / nb), ceil(2^32 / (2 nb))
+  unsigned int* ticket;                            // tile dispenser of this launch (device, zero before the launch)
 };
 
 // shared memory of one CTA: [rings: 16 warps x kSlots boxes][FsCtrl][binned: binS[2][nbins][64], lo/hi/r[nbins][128]]
@@ -73,6 +74,7 @@ struct __align__(16) FsCtrl {
   uint8_t lo[kFsCols], hi[kFsCols], rr[kFsCols];
   uint32_t T[kFsCols];                             // binned: per-column threshold on |nb x - S_b|
   uint64_t full[kFsWarps][4];                      // ring mbarriers
+  int tk[3][3];                                    // tile tickets handed to this CTA: {tile, beam, tile in beam}
 };
 __host__ __device__ inline size_t fd_stream_smem_bytes(int slots, int nbins_or_0) {
   size_t b = (size_t)kFsWarps * slots * kFsBoxWords * 4 + sizeof(FsCtrl);
@@ -141,23 +143,38 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
     for (int i = tid; i < 2 * P.nbins * (kFsCols / 2); i += kFsThreads) binS[i] = 0;
   __syncthreads();
 
-  // box `c` of tile `t` of this warp: rows [g RW + 8 c, + 8) of class cls of the tile's beam, x = first column
-  auto issue = [&](int64_t t, int c, int slot) {     // one lane
-    const int b = P.beam0 + (int)(t / P.tiles_per_beam);
-    const int s0 = (int)(t % P.tiles_per_beam) * kFsCols;
-    const int y = (int)(((int64_t)b * C) >> 2) + g * RW + kFsBoxRows * c;
+  // box `c` of a tile of this warp: rows [g RW + 8 c, + 8) of class cls of the tile's beam (y0 = the warp's first
+  // class row of that beam), x = the tile's first column
+  auto issue = [&](int s0, int y0, int c, int slot) {   // one lane
     mbar_arrive_expect_tx(&full[slot], kFsBoxWords * 4u);
-    fs_tma_load_2d(ring + slot * kFsBoxWords, &maps.src[cls], s0, y, &full[slot]);
+    fs_tma_load_2d(ring + slot * kFsBoxWords, &maps.src[cls], s0, y0 + kFsBoxRows * c, &full[slot]);
   };
-  const int64_t tstep = gridDim.x;
-  if (lane == 0 && (int64_t)blockIdx.x < P.total_tiles) {
+  // Tiles are handed out by a ticket counter, in order, two tickets ahead (the ring prefetches into the next tile).
+  // With a fixed stride the CTAs drift apart and the 64-byte DRAM atoms that neighbouring tiles share (a box row is
+  // the 144-byte superset of 128 columns of a 4-byte aligned row) are fetched twice: 18.7 GB of DRAM reads for a
+  // 9.2 GB batch.  Tickets keep neighbouring tiles in flight at the same time, so the second request hits L2.
+  auto take_ticket = [&](int slot_) {                 // one thread
+    const unsigned int t = atomicAdd(P.ticket, 1u);
+    const unsigned int tb = t / (unsigned int)P.tiles_per_beam;
+    K->tk[slot_][0] = (int)min(t, 0x7fffffffu);
+    K->tk[slot_][1] = (int)tb;
+    K->tk[slot_][2] = (int)(t - tb * (unsigned int)P.tiles_per_beam);
+  };
+  if (tid == 0) { take_ticket(0); take_ticket(1); }
+  __syncthreads();
+  int64_t cur_t = K->tk[0][0];
+  int cur_b = K->tk[0][1], cur_q = K->tk[0][2];
+  int64_t nxt_t = K->tk[1][0];
+  int nxt_b = K->tk[1][1], nxt_q = K->tk[1][2];
+  const int ywarp = g * RW;                           // + (beam * C) / 4: the warp's first class row of a beam
+  const int cq = C >> 2;
+  if (lane == 0 && cur_t < P.total_tiles) {
 #pragma unroll
     for (int c = 0; c < kSlots; ++c) {
       // NCH >= kSlots is guaranteed by the host
-      issue(blockIdx.x, c, c);
+      issue(cur_q * kFsCols, (P.beam0 + cur_b) * cq + ywarp, c, c);
     }
   }
-
   // binned: bit s of binend <=> this thread's block s is the last block of its bin; bin0 = bin of block 0.
   // (a block is 4 class rows = 16 channels; nb is a multiple of 16 and bins do not straddle warps: host-checked)
   uint32_t binend = 0;
@@ -176,9 +193,11 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
   uint32_t colS = 0, colQ = 0;                        // column owners (tid < 128): exact totals, kept across iterations
   const int offw = P.off[cls] >> 2;                   // word offset of column s0 inside a box row
 
-  for (int64_t t = blockIdx.x; t < P.total_tiles; t += tstep) {
-    const int b = P.beam0 + (int)(t / P.tiles_per_beam);
-    const int s0 = (int)(t % P.tiles_per_beam) * kFsCols;
+  while (cur_t < P.total_tiles) {
+    const int b = P.beam0 + cur_b;
+    const int s0 = cur_q * kFsCols;
+    const bool have_next = nxt_t < P.total_tiles;
+    const int nxt_s0 = nxt_q * kFsCols, nxt_y0 = (P.beam0 + nxt_b) * cq + ywarp, cur_y0 = b * cq + ywarp;
     const int tw = min(kFsCols, P.S - s0);            // valid columns of this tile
     const int nvalid = tw - 4 * lane;                 // valid bytes of this lane's word (>= 4: all)
     // row 0 of this warp's rows is channel 4 * (g RW) + cls; consecutive class rows are 4 channels apart
@@ -201,14 +220,6 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
       uint32_t w[kFsBoxRows];
 #pragma unroll
       for (int j = 0; j < kFsBoxRows; ++j) w[j] = rowp[j * kFsPitchW];
-      __syncwarp();                                   // every lane has its words: the box can be refilled
-      if (lane == 0) {
-        int cn = c + kSlots;
-        int64_t tn = t;
-        if (cn >= NCH) { cn -= NCH; tn = t + tstep; }
-        if (tn < P.total_tiles) issue(tn, cn, slot);
-      }
-      slot = (slot + 1 == kSlots) ? 0 : slot + 1;
       if (kCopy) {
         uint8_t* gd = dwarp + (int64_t)(kFsBoxRows * c) * rstep;
         if (nvalid >= 4) {
@@ -248,6 +259,15 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
           ++fbin;
         }
       }
+      // Refill the box only now: the statistics above have CONSUMED the eight words, so every lane's shared-memory
+      // loads have completed.  (Re-arming right after the loads were merely issued lets the asynchronous copy
+      // overtake them once the refill hits L2: a write-after-read hazard that showed up as rare wrong column sums.)
+      __syncwarp();
+      if (lane == 0) {
+        if (c + kSlots < NCH) issue(s0, cur_y0, c + kSlots, slot);                    // compile-time branch
+        else if (have_next) issue(nxt_s0, nxt_y0, c + kSlots - NCH, slot);
+      }
+      slot = (slot + 1 == kSlots) ? 0 : slot + 1;
     }
 #pragma unroll
     for (int u = 0; u < 4; ++u) {
@@ -256,11 +276,14 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
     }
 
     // ------------------------------------------------------------------ F3..F5: thresholds
+    int64_t nn_t = 0x7fffffff;
+    int nn_b = 0, nn_q = 0;
     for (int it = 0; it < P.n_thr; ++it) {
       const bool first = it == 0;
       const bool need_stats = it + 1 < P.n_thr;
       // ---- exchange: accumulators -> column owners -> bounds for everybody
       __syncthreads();                                                // A: accumulators (and bin sums) complete
+      if (first && tid == kFsThreads - 1) take_ticket(2);             // the tile after the next one
       if (tid < kFsCols) {
         const uint32_t q = K->acc[buf][kFsCols + tid];
         if (first) colQ = q; else colQ += q;                          // deltas are modulo 2^32
@@ -313,6 +336,7 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
         }
       }
       __syncthreads();                                                // B: bounds published
+      if (first) { nn_t = K->tk[2][0]; nn_b = K->tk[2][1]; nn_q = K->tk[2][2]; }
       if (tid < 2 * kFsCols) K->acc[buf][tid] = 0;                    // nobody reads this buffer any more
       buf ^= 1;
       if (kBinned && first) {                                         // the other bin-sum buffer is idle until the next tile
@@ -361,74 +385,149 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
         chiE = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4240u); cloE = 0x80008000u - prmt_b32(lo4, 0u, 0x4240u);
         chiO = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4341u); cloO = 0x80008000u - prmt_b32(lo4, 0u, 0x4341u);
       }
+      // Packed pre-test of a word against its four columns' kept intervals (two VIADDMNMX.U16x2): with neg = -lo and
+      // thr = hi - lo in the high byte of a u16 lane (low byte 0xff), (x + neg) mod 2^16 > thr <=> x outside [lo, hi].
+      // A column with an empty kept interval (lo > hi) cuts every value, which the packed form cannot say: `slow`.
+      uint32_t negE = 0, negO = 0, thrE = 0, thrO = 0;
+      bool slow = false;
+      auto packed_bounds = [&]() {
+        const uint32_t loE = prmt_b32(lo4, 0u, 0x2404u), loO = prmt_b32(lo4, 0u, 0x3414u);   // lo << 8 per u16 lane
+        const uint32_t hiE = prmt_b32(hi4, 0u, 0x2404u), hiO = prmt_b32(hi4, 0u, 0x3414u);
+        negE = __vsub2(0u, loE); negO = __vsub2(0u, loO);
+        thrE = __vsub2(hiE, loE) | 0x00ff00ffu; thrO = __vsub2(hiO, loO) | 0x00ff00ffu;
+        slow = __vcmpgtu4(lo4, hi4) != 0u;
+      };
+      auto word_hit = [&](uint32_t wv) {
+        return slow || __viaddmax_u16x2(wv, negO, thrO) != thrO || __viaddmax_u16x2(wv << 8, negE, thrE) != thrE;
+      };
+      if (!kBinned) packed_bounds();
       if (nvalid <= 0) hm = 0;
-      while (hm) {
-        const int s = __ffs(hm) - 1;
-        hm &= hm - 1;
-        int bin = 0;
-        if (kBinned) {
-          bin = bin0 + __popc(binend & ((1u << s) - 1u));             // bins that ended before block s
-          hi4 = reinterpret_cast<const uint32_t*>(hiB)[bin * (kFsCols / 4) + lane];
-          lo4 = reinterpret_cast<const uint32_t*>(loB)[bin * (kFsCols / 4) + lane];
-          r4 = reinterpret_cast<const uint32_t*>(rB)[bin * (kFsCols / 4) + lane];
-          chiE = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4240u); cloE = 0x80008000u - prmt_b32(lo4, 0u, 0x4240u);
-          chiO = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4341u); cloO = 0x80008000u - prmt_b32(lo4, 0u, 0x4341u);
-        }
-        uint8_t* gp = dwarp + (int64_t)(4 * s) * rstep;
-        uint32_t w[4];
-        if (nvalid >= 4) {
-#pragma unroll
-          for (int i = 0; i < 4; ++i) w[i] = *reinterpret_cast<const uint32_t*>(gp + i * rstep);
+      // One word of a candidate block: exact per-byte mask, replace in global memory, column (and bin) deltas.
+      uint32_t bsx01 = 0, bsx23 = 0;                                  // binned: packed signed deltas of the bin sums
+      auto fix_word = [&](uint32_t wv, uint8_t* gw, int ch, int nv) -> uint32_t {
+        uint32_t m = bytes_outside_cols(wv, chiE, cloE, chiO, cloO);
+        if (nv < 4) m &= (1u << (8 * nv)) - 1u;
+        if (m == 0) return wv;
+        const uint32_t nw = (wv & ~m) | (r4 & m);
+        if (nv >= 4) {
+          *reinterpret_cast<uint32_t*>(gw) = nw;
         } else {
+          for (int u = 0; u < nv; ++u) gw[u] = (uint8_t)(nw >> (8 * u));
+        }
+        const uint32_t f = wv & m;
+        cnt4 += m & 0x01010101u;
+        sq[0] = __dp4a(f & 0x000000ffu, f, sq[0]);
+        sq[1] = __dp4a(f & 0x0000ff00u, f, sq[1]);
+        sq[2] = __dp4a(f & 0x00ff0000u, f, sq[2]);
+        sq[3] = __dp4a(f & 0xff000000u, f, sq[3]);
+        if (!kBinned) {
+          sxE += prmt_b32(f, 0u, 0x4240u);
+          sxO += prmt_b32(f, 0u, 0x4341u);
+        } else {
+          // r - x per replaced byte, two columns per word: plain 32-bit arithmetic is exact here because the
+          // bin sums are back inside their 16-bit fields once all deltas of the iteration are in
+          const uint32_t rm = r4 & m;
+          bsx01 += (rm & 0xffu) - (f & 0xffu) + ((((rm >> 8) & 0xffu) - ((f >> 8) & 0xffu)) << 16);
+          bsx23 += ((rm >> 16) & 0xffu) - ((f >> 16) & 0xffu) + (((rm >> 24) - (f >> 24)) << 16);
+          rq[0] = __dp4a(rm & 0x000000ffu, rm, rq[0]);                // r differs from bin to bin
+          rq[1] = __dp4a(rm & 0x0000ff00u, rm, rq[1]);
+          rq[2] = __dp4a(rm & 0x00ff0000u, rm, rq[2]);
+          rq[3] = __dp4a(rm & 0xff000000u, rm, rq[3]);
+        }
+        if (P.flags) {
+          uint8_t* fl = P.flags + ((int64_t)b * C + ch) * P.S + s0 + 4 * lane;
 #pragma unroll
+          for (int u = 0; u < 4; ++u)
+            if ((m >> (8 * u)) & 1u) fl[u] = 1;
+        }
+        return nw;
+      };
+      if (nvalid >= 4) {
+        // The next candidate's four words are requested before the current block is examined: the blocks are
+        // distinct, and a warp's trip count is the largest candidate count among its lanes, so the L2 round trip
+        // is what a trip costs otherwise.
+        uint32_t wn[4] = {0, 0, 0, 0};
+        int sn = -1;
+        if (hm) {
+          sn = __ffs(hm) - 1;
+          hm &= hm - 1;
+          const uint8_t* gp = dwarp + (int64_t)(4 * sn) * rstep;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) wn[i] = *reinterpret_cast<const uint32_t*>(gp + i * rstep);
+        }
+        while (sn >= 0) {
+          const int s = sn;
+          const uint32_t w0 = wn[0], w1 = wn[1], w2 = wn[2], w3 = wn[3];
+          sn = -1;
+          if (hm) {
+            sn = __ffs(hm) - 1;
+            hm &= hm - 1;
+            const uint8_t* gp = dwarp + (int64_t)(4 * sn) * rstep;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) wn[i] = *reinterpret_cast<const uint32_t*>(gp + i * rstep);
+          }
+          int bin = 0;
+          if (kBinned) {
+            bin = bin0 + __popc(binend & ((1u << s) - 1u));           // bins that ended before block s
+            hi4 = reinterpret_cast<const uint32_t*>(hiB)[bin * (kFsCols / 4) + lane];
+            lo4 = reinterpret_cast<const uint32_t*>(loB)[bin * (kFsCols / 4) + lane];
+            r4 = reinterpret_cast<const uint32_t*>(rB)[bin * (kFsCols / 4) + lane];
+            chiE = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4240u); cloE = 0x80008000u - prmt_b32(lo4, 0u, 0x4240u);
+            chiO = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4341u); cloO = 0x80008000u - prmt_b32(lo4, 0u, 0x4341u);
+            bsx01 = 0; bsx23 = 0;
+            packed_bounds();
+          }
+          const bool h0 = word_hit(w0), h1 = word_hit(w1), h2 = word_hit(w2), h3 = word_hit(w3);
+          if (h0 | h1 | h2 | h3) {
+            uint8_t* gp = dwarp + (int64_t)(4 * s) * rstep;
+            const int ch = 4 * (g * RW + 4 * s) + cls;
+            uint32_t n0 = w0, n1 = w1, n2 = w2, n3 = w3;
+            if (h0) n0 = fix_word(w0, gp, ch, 4);
+            if (h1) n1 = fix_word(w1, gp + rstep, ch + 4, 4);
+            if (h2) n2 = fix_word(w2, gp + 2 * rstep, ch + 8, 4);
+            if (h3) n3 = fix_word(w3, gp + 3 * rstep, ch + 12, 4);
+            if (kBinned && need_stats && (bsx01 | bsx23)) {
+              fs_red_add(&bS[bin * (kFsCols / 2) + 2 * lane], bsx01);
+              fs_red_add(&bS[bin * (kFsCols / 2) + 2 * lane + 1], bsx23);
+            }
+            if (need_stats) {
+              // a later iteration should not examine this block again for what has just been replaced: refresh its
+              // summary (byte s & 3 of register s >> 2; the register index is resolved by predication)
+              const uint32_t e = group_summary(make_uint4(n0, n1, n2, n3));
+              const int sh = 4 * (s & 3);
+              const uint32_t selx = (0x3210u & ~(0xfu << sh)) | (0x5u << sh);
+              const uint32_t seln = (0x3210u & ~(0xfu << sh)) | (0x4u << sh);
+#pragma unroll
+              for (int i = 0; i < NREG; ++i)
+                if ((s >> 2) == i) { MX[i] = prmt(MX[i], e, selx); MN[i] = prmt(MN[i], e, seln); }
+            }
+          }
+        }
+      } else {
+        // the last word of a row with 1..3 valid bytes: byte-granular loads and stores
+        while (hm) {
+          const int s = __ffs(hm) - 1;
+          hm &= hm - 1;
+          int bin = 0;
+          if (kBinned) {
+            bin = bin0 + __popc(binend & ((1u << s) - 1u));
+            hi4 = reinterpret_cast<const uint32_t*>(hiB)[bin * (kFsCols / 4) + lane];
+            lo4 = reinterpret_cast<const uint32_t*>(loB)[bin * (kFsCols / 4) + lane];
+            r4 = reinterpret_cast<const uint32_t*>(rB)[bin * (kFsCols / 4) + lane];
+            chiE = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4240u); cloE = 0x80008000u - prmt_b32(lo4, 0u, 0x4240u);
+            chiO = 0x7fff7fffu - prmt_b32(hi4, 0u, 0x4341u); cloO = 0x80008000u - prmt_b32(lo4, 0u, 0x4341u);
+            bsx01 = 0; bsx23 = 0;
+          }
+          uint8_t* gp = dwarp + (int64_t)(4 * s) * rstep;
           for (int i = 0; i < 4; ++i) {
-            w[i] = 0;
-            for (int u = 0; u < nvalid; ++u) w[i] |= (uint32_t)gp[i * rstep + u] << (8 * u);
+            uint32_t wv = 0;
+            for (int u = 0; u < nvalid; ++u) wv |= (uint32_t)gp[i * rstep + u] << (8 * u);
+            fix_word(wv, gp + i * rstep, 4 * (g * RW + 4 * s + i) + cls, nvalid);
           }
-        }
-        uint32_t bsx01 = 0, bsx23 = 0;                                // binned: packed signed deltas of the bin sums
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          uint32_t m = bytes_outside_cols(w[i], chiE, cloE, chiO, cloO);
-          if (nvalid < 4) m &= (1u << (8 * nvalid)) - 1u;
-          if (m == 0) continue;
-          const uint32_t nw = (w[i] & ~m) | (r4 & m);
-          if (nvalid >= 4) {
-            *reinterpret_cast<uint32_t*>(gp + i * rstep) = nw;
-          } else {
-            for (int u = 0; u < nvalid; ++u) gp[i * rstep + u] = (uint8_t)(nw >> (8 * u));
+          if (kBinned && need_stats && (bsx01 | bsx23)) {
+            fs_red_add(&bS[bin * (kFsCols / 2) + 2 * lane], bsx01);
+            fs_red_add(&bS[bin * (kFsCols / 2) + 2 * lane + 1], bsx23);
           }
-          const uint32_t f = w[i] & m;
-          cnt4 += m & 0x01010101u;
-          sq[0] = __dp4a(f & 0x000000ffu, f, sq[0]);
-          sq[1] = __dp4a(f & 0x0000ff00u, f, sq[1]);
-          sq[2] = __dp4a(f & 0x00ff0000u, f, sq[2]);
-          sq[3] = __dp4a(f & 0xff000000u, f, sq[3]);
-          if (!kBinned) {
-            sxE += prmt_b32(f, 0u, 0x4240u);
-            sxO += prmt_b32(f, 0u, 0x4341u);
-          } else {
-            // r - x per replaced byte, two columns per word: plain 32-bit arithmetic is exact here because the
-            // bin sums are back inside their 16-bit fields once all deltas of the iteration are in
-            const uint32_t rm = r4 & m;
-            bsx01 += (rm & 0xffu) - (f & 0xffu) + ((((rm >> 8) & 0xffu) - ((f >> 8) & 0xffu)) << 16);
-            bsx23 += ((rm >> 16) & 0xffu) - ((f >> 16) & 0xffu) + (((rm >> 24) - (f >> 24)) << 16);
-            rq[0] = __dp4a(rm & 0x000000ffu, rm, rq[0]);              // r differs from bin to bin
-            rq[1] = __dp4a(rm & 0x0000ff00u, rm, rq[1]);
-            rq[2] = __dp4a(rm & 0x00ff0000u, rm, rq[2]);
-            rq[3] = __dp4a(rm & 0xff000000u, rm, rq[3]);
-          }
-          if (P.flags) {
-            const int ch = 4 * (g * RW + 4 * s + i) + cls;
-            uint8_t* fl = P.flags + ((int64_t)b * C + ch) * P.S + s0 + 4 * lane;
-#pragma unroll
-            for (int u = 0; u < 4; ++u)
-              if ((m >> (8 * u)) & 1u) fl[u] = 1;
-          }
-        }
-        if (kBinned && need_stats && (bsx01 | bsx23)) {
-          fs_red_add(&bS[bin * (kFsCols / 2) + 2 * lane], bsx01);
-          fs_red_add(&bS[bin * (kFsCols / 2) + 2 * lane + 1], bsx23);
         }
       }
       if ((need_stats || P.counts) && __any_sync(FULL, cnt4 != 0u)) {
@@ -454,6 +553,8 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
       }
     }
     bsel ^= 1;
+    cur_t = nxt_t; cur_b = nxt_b; cur_q = nxt_q;
+    nxt_t = nn_t; nxt_b = nn_b; nxt_q = nn_q;
   }
 }
 

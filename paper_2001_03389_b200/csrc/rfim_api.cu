@@ -149,6 +149,7 @@ int validate(int op, void* data, int beams, int channels, int samples, rfim_dtyp
   c.counts = reinterpret_cast<unsigned long long*>(z.counts);
   c.stream = reinterpret_cast<cudaStream_t>(z.stream);
   c.workspace = z.workspace;
+  if (z.workspace && (reinterpret_cast<uintptr_t>(z.workspace) & 255) != 0) return RFIM_ERR_INVALID;
   c.variant = z.variant;
   c.reserved_team = 0;
   c.keep_outputs = false;
@@ -358,11 +359,14 @@ EncodeTiledFn encode_tiled_fn() {
 // remembered per thread: a real-time caller cleans the same buffers batch after batch.
 struct ClassMaps { CUtensorMap m[4]; int off[4]; };
 bool encode_class_maps(const uint8_t* base, int64_t stride, int samples, int64_t rows, int box_w, int box_rows,
-                       ClassMaps& out) {
-  struct Key { const uint8_t* base; int64_t stride; int samples; int64_t rows; int box_w, box_rows; };
-  thread_local Key last_key = {nullptr, 0, 0, 0, 0, 0};
+                       CUtensorMapL2promotion promo, ClassMaps& out) {
+  struct Key { const uint8_t* base; int64_t stride; int samples; int64_t rows; int box_w, box_rows, promo; };
+  thread_local Key last_key = {nullptr, 0, 0, 0, 0, 0, 0};
   thread_local ClassMaps last_maps;
-  const Key key = {base, stride, samples, rows, box_w, box_rows};
+  Key key;
+  memset(&key, 0, sizeof(key));
+  key.base = base; key.stride = stride; key.samples = samples; key.rows = rows; key.box_w = box_w;
+  key.box_rows = box_rows; key.promo = (int)promo;
   if (last_key.base != nullptr && memcmp(&last_key, &key, sizeof(Key)) == 0) { out = last_maps; return true; }
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
@@ -374,11 +378,10 @@ bool encode_class_maps(const uint8_t* base, int64_t stride, int samples, int64_t
     cuuint32_t box[2] = {(cuuint32_t)box_w, (cuuint32_t)box_rows};
     cuuint32_t estr[2] = {1, 1};
     if (enc(&out.m[k], CU_TENSOR_MAP_DATA_TYPE_UINT8, 2, reinterpret_cast<void*>(addr - out.off[k]), dims, strides,
-            box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, CU_TENSOR_MAP_L2_PROMOTION_L2_128B,
+            box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE, promo,
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return false;
   }
-  memset(&last_key, 0, sizeof(Key));
   last_key = key;
   last_maps = out;
   return true;
@@ -404,6 +407,7 @@ bool plan_fd_u8_stream(const Call& c, StreamPlan& pl) {
     pl.nbins = c.channels / nb;
     if (pl.nbins > rfim::kFsMaxBins) return false;
   }
+  if ((int64_t)c.beams * ((c.samples + rfim::kFsCols - 1) / rfim::kFsCols) >= 0x7fffffff) return false;   // tickets
   pl.copy = c.out != c.data;
   pl.slots = pl.binned ? 3 : 4;
   pl.smem = (int)rfim::fd_stream_smem_bytes(pl.slots, pl.nbins);
@@ -430,7 +434,29 @@ int launch_fd_stream_n(const Call& c, const StreamPlan& pl, const rfim::FdStream
   int64_t grid = P.total_tiles;
   if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
   if ((st = clear_outputs(c)) != RFIM_OK) return st;
-  return launch(name, kernel, dim3((unsigned)grid), dim3(rfim::kFsThreads), (size_t)pl.smem, c.stream, 0, maps, P);
+  // the tile dispenser: 4 bytes of zeroed device memory, the caller's (opts->workspace) or, failing that, taken from
+  // and returned to the stream-ordered memory pool around the launch
+  rfim::FdStreamParams Q = P;
+  bool owned = false;
+  if (c.workspace) {
+    Q.ticket = static_cast<unsigned int*>(c.workspace);
+  } else {
+    void* p = nullptr;
+    CUDA_TRY(cudaMallocAsync(&p, 256, c.stream));
+    Q.ticket = static_cast<unsigned int*>(p);
+    owned = true;
+  }
+  cudaError_t e = cudaMemsetAsync(Q.ticket, 0, sizeof(unsigned int), c.stream);
+  if (e != cudaSuccess) {
+    if (owned) cudaFreeAsync(Q.ticket, c.stream);
+    return cuda_fail(e, "cudaMemsetAsync(ticket)");
+  }
+  st = launch(name, kernel, dim3((unsigned)grid), dim3(rfim::kFsThreads), (size_t)pl.smem, c.stream, 0, maps, Q);
+  if (owned) {
+    e = cudaFreeAsync(Q.ticket, c.stream);
+    if (e != cudaSuccess && st == RFIM_OK) st = cuda_fail(e, "cudaFreeAsync(ticket)");
+  }
+  return st;
 }
 
 int launch_fd_stream(const Call& c, const StreamPlan& pl, int sms) {
@@ -453,8 +479,12 @@ int launch_fd_stream(const Call& c, const StreamPlan& pl, int sms) {
   P.inv_nb = (uint32_t)((((uint64_t)1 << 32) + (uint64_t)P.nb - 1) / (uint64_t)P.nb);
   P.inv_2nb = (uint32_t)((((uint64_t)1 << 32) + 2 * (uint64_t)P.nb - 1) / (2 * (uint64_t)P.nb));
   ClassMaps cm;
+  // No L2 promotion: a box row is the 144-byte superset of 128 columns; promoted to whole 128-byte lines it costs
+  // two lines (256 bytes) of DRAM traffic, because the half-used line is rarely still in L2 when the neighbouring
+  // tile asks for it (measured: 18.2 GB read for a 9.2 GB batch with 128-byte promotion).
+  const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_NONE;
   if (!encode_class_maps(P.src, c.stride, c.samples, (int64_t)c.beams * c.channels, rfim::kFsPitchW * 4,
-                         rfim::kFsBoxRows, cm))
+                         rfim::kFsBoxRows, promo, cm))
     return RFIM_ERR_UNSUPPORTED;
   rfim::FdStreamMaps maps;
   for (int k = 0; k < 4; ++k) { maps.src[k] = cm.m[k]; P.off[k] = cm.off[k]; }
@@ -531,7 +561,7 @@ int launch_fd_strip(const Call& c, const StripPlan& pl, int sms) {
   if (pl.tensor) {
     ClassMaps cm;
     if (!encode_class_maps(P.src, c.stride, c.samples, (int64_t)c.beams * c.channels, rfim::kStripPitchW * 4,
-                           pl.box_rows, cm))
+                           pl.box_rows, CU_TENSOR_MAP_L2_PROMOTION_L2_128B, cm))
       return RFIM_ERR_UNSUPPORTED;
     for (int k = 0; k < 4; ++k) { maps.src[k] = cm.m[k]; P.off[k] = cm.off[k]; }
     P.box_rows = pl.box_rows;
@@ -834,8 +864,8 @@ int rfim_sigma_cut_host(void* data, void* out, int beams, int channels, int samp
                                             (size_t)samples * es, rows, cudaMemcpyHostToDevice, s);
     if (e != cudaSuccess) { fail(e, stride == samples ? "cudaMemcpyAsync(H2D)" : "cudaMemcpy2DAsync(H2D)"); break; }
     Call t = ct, f = cf;
-    t.data = t.out = dev[slot]; t.beams = nb; t.stream = s;
-    if (n_freq > 0) { f.data = f.out = dev[slot]; f.beams = nb; f.stream = s; }
+    t.data = t.out = dev[slot]; t.beams = nb; t.stream = s; t.workspace = nullptr;
+    if (n_freq > 0) { f.data = f.out = dev[slot]; f.beams = nb; f.stream = s; f.workspace = nullptr; }
     if (n_time > 0) {
       if ((st = run_time(t)) != RFIM_OK) { rc = st; break; }
     }
@@ -859,7 +889,8 @@ int rfim_sigma_cut_host(void* data, void* out, int beams, int channels, int samp
 size_t rfim_workspace_bytes(int op, int beams, int channels, int samples, rfim_dtype dtype,
                             int n_thresholds, rfim_replace policy, const rfim_opts* opts) {
   (void)n_thresholds; (void)policy;
-  if (op != RFIM_OP_HOST) return 0;                   // the device entry points need no scratch today
+  if (op == RFIM_OP_FREQ || op == RFIM_OP_TIME_FREQ) return 256;   // the FDSC tile dispenser (4 bytes used)
+  if (op != RFIM_OP_HOST) return 0;                   // TDSC needs no scratch
   if (beams <= 0 || channels <= 0 || samples <= 0 || (dtype != RFIM_U8 && dtype != RFIM_F32)) return 0;
   const size_t es = elem_size(dtype);
   int64_t stride = (opts && opts->sample_stride) ? opts->sample_stride : samples;

@@ -120,11 +120,12 @@ def test_host_path_validates_only_what_runs():
 
 
 def test_workspace_bytes():
-    """Device entry points need no scratch; the host path needs its three staging buffers (chunks of whole beams of
-    about 128 MiB, rounded up to 256 bytes), fewer when there are fewer chunks."""
+    """TDSC needs no scratch, FDSC 256 bytes (the tile dispenser of the streaming kernel); the host path needs its
+    three staging buffers (chunks of whole beams of about 128 MiB, rounded up to 256 bytes), fewer when there are
+    fewer chunks."""
     assert rfim.rfim_workspace_bytes(rfim.OP_TIME, 480, 1536, 12500) == 0
-    assert rfim.rfim_workspace_bytes(rfim.OP_FREQ, 480, 1536, 12500) == 0
-    assert rfim.rfim_workspace_bytes(rfim.OP_TIME_FREQ, 480, 1536, 12500) == 0
+    assert rfim.rfim_workspace_bytes(rfim.OP_FREQ, 480, 1536, 12500) == 256
+    assert rfim.rfim_workspace_bytes(rfim.OP_TIME_FREQ, 480, 1536, 12500) == 256
     beam = 1536 * 12500
     per_chunk = (128 << 20) // beam
     assert per_chunk == 6
