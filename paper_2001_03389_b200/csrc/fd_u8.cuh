@@ -7,6 +7,7 @@
 #pragma once
 
 #include "common.cuh"
+#include "packed.cuh"
 
 namespace rfim {
 
@@ -21,58 +22,6 @@ struct FdU8Params {
   uint8_t* flags;               // optional [beams][C][S]
   unsigned long long* counts;   // optional [n_thr]
 };
-
-__device__ __forceinline__ uint32_t prmt_b32(uint32_t a, uint32_t b, uint32_t sel) {
-  uint32_t d;
-  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));
-  return d;
-}
-
-// ---------------------------------------------------------------- cluster helpers
-__device__ __forceinline__ uint32_t cluster_ctarank() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
-  return r;
-}
-__device__ __forceinline__ uint32_t cluster_nctarank() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%cluster_nctarank;" : "=r"(r));
-  return r;
-}
-__device__ __forceinline__ uint32_t cluster_id_x() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%clusterid.x;" : "=r"(r));
-  return r;
-}
-__device__ __forceinline__ uint32_t cluster_nid_x() {
-  uint32_t r;
-  asm volatile("mov.u32 %0, %%nclusterid.x;" : "=r"(r));
-  return r;
-}
-// barrier over all threads of all CTAs of the cluster; orders shared-memory accesses cluster-wide
-__device__ __forceinline__ void cluster_sync_all() {
-  asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
-}
-// address of the same shared-memory location in CTA `rank` of the cluster
-__device__ __forceinline__ uint32_t dsmem_addr(const void* local, uint32_t rank) {
-  uint32_t ra;
-  asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(ra) : "r"(smem_addr(local)), "r"(rank));
-  return ra;
-}
-__device__ __forceinline__ uint32_t dsmem_ld_u32(uint32_t addr) {
-  uint32_t v;
-  asm volatile("ld.shared::cluster.u32 %0, [%1];" : "=r"(v) : "r"(addr));
-  return v;
-}
-// Exact 0xFF-per-byte mask of the bytes of w outside their column's [lo, hi]; constants per u16 lane:
-// chiE/cloE for bytes 0 and 2, chiO/cloO for bytes 1 and 3 (see bytes_outside in td_u8.cuh).
-__device__ __forceinline__ uint32_t bytes_outside_cols(uint32_t w, uint32_t chiE, uint32_t cloE, uint32_t chiO,
-                                                       uint32_t cloO) {
-  const uint32_t xe = prmt_b32(w, 0u, 0x4240u), xo = prmt_b32(w, 0u, 0x4341u);
-  const uint32_t fe = (xe + chiE) | ~(xe + cloE);
-  const uint32_t fo = (xo + chiO) | ~(xo + cloO);
-  return prmt_b32(fe, fo, 0xFBD9u);
-}
 
 // ---------------------------------------------------------------- generic kernel
 constexpr int kFdGenericThreads = 128;

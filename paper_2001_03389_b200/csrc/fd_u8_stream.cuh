@@ -32,8 +32,7 @@
 #include <cuda.h>   // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
 
 #include "common.cuh"
-#include "fd_u8.cuh"
-#include "td_u8.cuh"   // prmt, group_summary, bytes_above, bytes_below
+#include "packed.cuh"
 
 namespace rfim {
 

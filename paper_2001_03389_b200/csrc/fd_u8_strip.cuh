@@ -28,7 +28,7 @@
 #include <cuda.h>   // CUtensorMap (types only: the encoder is fetched through the runtime, no -lcuda)
 
 #include "common.cuh"
-#include "fd_u8.cuh"
+#include "packed.cuh"
 
 namespace rfim {
 

@@ -1,0 +1,87 @@
+// launch_fd_misc.cu -- variant selection over the FDSC uint8 kernel families, and the launches of the correctness
+// paths (fd_u8.cuh, fd_u8_binned.cuh, fd_f32.cuh).
+#include "host.h"
+#include "fd_u8.cuh"
+#include "fd_f32.cuh"
+#include "fd_u8_binned.cuh"
+
+namespace rfim_host {
+
+int launch_fd_u8(const Call& c) {
+  int sms = 0;
+  int st = sm_count(sms);
+  if (st != RFIM_OK) return st;
+
+  // 0 = auto, 2 = any tuned kernel, 16 = the streaming kernel
+  if (c.variant == 0 || c.variant == 2 || c.variant == 16) {
+    st = try_fd_u8_stream(c, sms);
+    if (st != RFIM_ERR_UNSUPPORTED) return st;
+    if (c.variant == 16) return RFIM_ERR_UNSUPPORTED;
+  }
+  // 13: strip kernel with per-row bulk copies; 14: never the single-CTA tile; 15: the strip kernel
+  if (c.variant == 0 || c.variant == 2 || (c.variant >= 13 && c.variant <= 15)) {
+    st = try_fd_u8_strip(c, c.variant != 13, c.variant == 14 ? -1 : 0, sms);
+    if (st != RFIM_ERR_UNSUPPORTED) return st;
+  }
+  if (c.variant >= 2) return RFIM_ERR_UNSUPPORTED;
+
+  if (c.bin_size != c.channels || c.policy == RFIM_REPLACE_MEDIAN) {   // per-bin mean correction and / or median
+    rfim::FdBinnedParams B;                                             // replacement: correctness path
+    memset(&B, 0, sizeof(B));
+    B.src = static_cast<const uint8_t*>(c.data); B.dst = static_cast<uint8_t*>(c.out); B.stride = c.stride;
+    B.beams = c.beams; B.C = c.channels; B.S = c.samples; B.nb = c.bin_size;
+    B.n_thr = c.n_thr;
+    B.policy = (int)c.policy;
+    for (int i = 0; i < c.n_thr; ++i) B.p[i] = quantise(c.thr[i]);
+    B.flags = c.flags; B.counts = c.counts;
+    const int64_t ncol = (int64_t)c.beams * c.samples;
+    int64_t grid = (ncol + rfim::kFdBinnedThreads - 1) / rfim::kFdBinnedThreads;
+    if (grid > (int64_t)sms * 16) grid = (int64_t)sms * 16;
+    if ((st = clear_outputs(c)) != RFIM_OK) return st;
+    return launch("fd_u8_binned_generic", rfim::fd_u8_binned_kernel, dim3((unsigned)grid),
+                  dim3(rfim::kFdBinnedThreads), 0, c.stream, 0, B);
+  }
+  rfim::FdU8Params P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const uint8_t*>(c.data);
+  P.dst = static_cast<uint8_t*>(c.out);
+  P.stride = c.stride;
+  P.beams = c.beams; P.C = c.channels; P.S = c.samples;
+  P.n_thr = c.n_thr;
+  for (int i = 0; i < c.n_thr; ++i) { P.p[i] = quantise(c.thr[i]); P.pf[i] = (float)P.p[i] * (1.0f / 65536.0f); }
+  P.flags = c.flags;
+  P.counts = c.counts;
+  const int64_t ncol = (int64_t)c.beams * c.samples;
+  int64_t grid = (ncol + rfim::kFdGenericThreads - 1) / rfim::kFdGenericThreads;
+  if (grid > (int64_t)sms * 16) grid = (int64_t)sms * 16;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  return launch("fd_u8_generic", rfim::fd_u8_generic_kernel, dim3((unsigned)grid), dim3(rfim::kFdGenericThreads), 0,
+                c.stream, 0, P);
+}
+
+// ------------------------------------------------------------------------------------------ FD f32
+int launch_fd_f32(const Call& c) {
+  rfim::FdF32Params P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const float*>(c.data);
+  P.dst = static_cast<float*>(c.out);
+  P.stride = c.stride;
+  P.beams = c.beams; P.C = c.channels; P.S = c.samples; P.nb = c.bin_size;
+  P.n_thr = c.n_thr;
+  P.policy = (int)c.policy;
+  for (int i = 0; i < c.n_thr; ++i) P.k[i] = c.thr[i];
+  P.flags = c.flags;
+  P.counts = c.counts;
+  if (c.variant >= 2) return RFIM_ERR_UNSUPPORTED;                 // only the correctness path exists
+  int sms = 0;
+  int st = sm_count(sms);
+  if (st != RFIM_OK) return st;
+  const int64_t ncol = (int64_t)c.beams * c.samples;
+  int64_t grid = (ncol + rfim::kFdF32Threads - 1) / rfim::kFdF32Threads;
+  if (grid > (int64_t)sms * 16) grid = (int64_t)sms * 16;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  return launch("fd_f32_generic", rfim::fd_f32_generic_kernel, dim3((unsigned)grid), dim3(rfim::kFdF32Threads), 0,
+                c.stream, 0, P);
+}
+
+}  // namespace rfim_host

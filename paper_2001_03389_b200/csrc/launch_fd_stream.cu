@@ -1,0 +1,122 @@
+// launch_fd_stream.cu -- geometry and launch of the streaming FDSC uint8 kernel (fd_u8_stream.cuh).
+#include "host.h"
+#include "fd_u8_stream.cuh"
+
+namespace rfim_host {
+
+// ---- streaming kernel (fd_u8_stream.cuh): channel counts of 128 * {4, 8, 12, 16}, mean replacement, one bin or
+// bins whose size is a multiple of 16 that divides the 32 * NCH channels one warp quartet owns
+struct StreamPlan { int nch, slots, smem, nbins; bool binned, copy; };
+bool plan_fd_u8_stream(const Call& c, StreamPlan& pl) {
+  if (c.policy != RFIM_REPLACE_MEAN) return false;
+  if (c.channels % 128 != 0) return false;
+  pl.nch = c.channels / 128;
+  if (pl.nch != 4 && pl.nch != 8 && pl.nch != 12 && pl.nch != 16) return false;
+  const uintptr_t src = reinterpret_cast<uintptr_t>(c.data), dst = reinterpret_cast<uintptr_t>(c.out);
+  if ((src & 3) != 0 || (dst & 3) != 0 || (c.stride & 3) != 0) return false;     // 32-bit word columns
+  if ((int64_t)c.beams * c.channels / 4 > 0x7fffffff) return false;              // tensor coordinates
+  if (!tensor_maps_available()) return false;
+  pl.binned = c.bin_size != c.channels;
+  pl.nbins = 0;
+  if (pl.binned) {
+    const int nb = c.bin_size;
+    if (nb % 16 != 0 || nb > 256 || (32 * pl.nch) % nb != 0) return false;
+    pl.nbins = c.channels / nb;
+    if (pl.nbins > rfim::kFsMaxBins) return false;
+  }
+  if ((int64_t)c.beams * ((c.samples + rfim::kFsCols - 1) / rfim::kFsCols) >= 0x7fffffff) return false;   // tickets
+  pl.copy = c.out != c.data;
+  pl.slots = pl.binned ? 3 : 4;
+  pl.smem = (int)rfim::fd_stream_smem_bytes(pl.slots, pl.nbins);
+  return pl.smem <= kMaxSmem;
+}
+
+template <int NCH>
+int launch_fd_stream_n(const Call& c, const StreamPlan& pl, const rfim::FdStreamMaps& maps,
+                       const rfim::FdStreamParams& P, int sms) {
+  void (*kernel)(const rfim::FdStreamMaps, const rfim::FdStreamParams);
+  const char* name;
+  if (pl.binned) {
+    kernel = pl.copy ? rfim::fd_u8_stream_kernel<NCH, 3, true, true> : rfim::fd_u8_stream_kernel<NCH, 3, true, false>;
+    name = pl.copy ? "fd_u8_stream_binned_copy" : "fd_u8_stream_binned";
+  } else {
+    kernel = pl.copy ? rfim::fd_u8_stream_kernel<NCH, 4, false, true> : rfim::fd_u8_stream_kernel<NCH, 4, false, false>;
+    name = pl.copy ? "fd_u8_stream_copy" : "fd_u8_stream";
+  }
+  int st = ensure_smem(kernel, (size_t)pl.smem);
+  if (st != RFIM_OK) return st;
+  int occ = 0;
+  if ((st = blocks_per_sm(kernel, rfim::kFsThreads, (size_t)pl.smem, occ)) != RFIM_OK) return st;
+  if (occ < 1) return RFIM_ERR_UNSUPPORTED;
+  int64_t grid = P.total_tiles;
+  if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  // the tile dispenser: 4 bytes of zeroed device memory, the caller's (opts->workspace) or, failing that, taken from
+  // and returned to the stream-ordered memory pool around the launch
+  rfim::FdStreamParams Q = P;
+  bool owned = false;
+  if (c.workspace) {
+    Q.ticket = static_cast<unsigned int*>(c.workspace);
+  } else {
+    void* p = nullptr;
+    CUDA_TRY(cudaMallocAsync(&p, 256, c.stream));
+    Q.ticket = static_cast<unsigned int*>(p);
+    owned = true;
+  }
+  cudaError_t e = cudaMemsetAsync(Q.ticket, 0, sizeof(unsigned int), c.stream);
+  if (e != cudaSuccess) {
+    if (owned) cudaFreeAsync(Q.ticket, c.stream);
+    return cuda_fail(e, "cudaMemsetAsync(ticket)");
+  }
+  st = launch(name, kernel, dim3((unsigned)grid), dim3(rfim::kFsThreads), (size_t)pl.smem, c.stream, 0, maps, Q);
+  if (owned) {
+    e = cudaFreeAsync(Q.ticket, c.stream);
+    if (e != cudaSuccess && st == RFIM_OK) st = cuda_fail(e, "cudaFreeAsync(ticket)");
+  }
+  return st;
+}
+
+int launch_fd_stream(const Call& c, const StreamPlan& pl, int sms) {
+  rfim::FdStreamParams P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const uint8_t*>(c.data);
+  P.dst = static_cast<uint8_t*>(c.out);
+  P.stride = c.stride;
+  P.beams = c.beams; P.C = c.channels; P.S = c.samples;
+  P.beam0 = 0;
+  P.n_thr = c.n_thr;
+  for (int i = 0; i < c.n_thr; ++i) P.p[i] = quantise(c.thr[i]);
+  P.flags = c.flags;
+  P.counts = c.counts;
+  P.tiles_per_beam = (c.samples + rfim::kFsCols - 1) / rfim::kFsCols;
+  P.total_tiles = (int64_t)P.tiles_per_beam * c.beams;
+  P.invC = (uint32_t)((((uint64_t)1 << 32) + (uint64_t)c.channels - 1) / (uint64_t)c.channels);
+  P.nb = c.bin_size;
+  P.nbins = pl.nbins;
+  P.inv_nb = (uint32_t)((((uint64_t)1 << 32) + (uint64_t)P.nb - 1) / (uint64_t)P.nb);
+  P.inv_2nb = (uint32_t)((((uint64_t)1 << 32) + 2 * (uint64_t)P.nb - 1) / (2 * (uint64_t)P.nb));
+  ClassMaps cm;
+  // No L2 promotion: a box row is the 144-byte superset of 128 columns; promoted to whole 128-byte lines it costs
+  // two lines (256 bytes) of DRAM traffic, because the half-used line is rarely still in L2 when the neighbouring
+  // tile asks for it (measured: 18.2 GB read for a 9.2 GB batch with 128-byte promotion).
+  const CUtensorMapL2promotion promo = CU_TENSOR_MAP_L2_PROMOTION_NONE;
+  if (!encode_class_maps(P.src, c.stride, c.samples, (int64_t)c.beams * c.channels, rfim::kFsPitchW * 4,
+                         rfim::kFsBoxRows, promo, cm))
+    return RFIM_ERR_UNSUPPORTED;
+  rfim::FdStreamMaps maps;
+  for (int k = 0; k < 4; ++k) { maps.src[k] = cm.m[k]; P.off[k] = cm.off[k]; }
+  switch (pl.nch) {
+    case 4: return launch_fd_stream_n<4>(c, pl, maps, P, sms);
+    case 8: return launch_fd_stream_n<8>(c, pl, maps, P, sms);
+    case 12: return launch_fd_stream_n<12>(c, pl, maps, P, sms);
+    default: return launch_fd_stream_n<16>(c, pl, maps, P, sms);
+  }
+}
+
+int try_fd_u8_stream(const Call& c, int sms) {
+  StreamPlan sp;
+  if (!plan_fd_u8_stream(c, sp)) return RFIM_ERR_UNSUPPORTED;
+  return launch_fd_stream(c, sp, sms);
+}
+
+}  // namespace rfim_host
