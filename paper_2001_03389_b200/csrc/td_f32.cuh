@@ -8,8 +8,9 @@
 //   the pitch is a multiple of 4; otherwise by coalesced loads).  The CTA's warps form TEAMS of kTW
 //   warps; a team owns one window at a time.
 //   T2: one pass, fp64: A = sum (x - c), B = sum (x - c)^2 around the pivot c = x[0] of the window
-//       (mu = c + A/N, sigma^2 = B/N - (A/N)^2: no cancellation to speak of, because |A/N| is of the
-//       order of sigma).
+//       (mu = c + A/N, sigma^2 = B/N - (A/N)^2); when the pivot turns out to be far from the mean in units
+//       of sigma (a spike at x[0], or after a huge sample was replaced) the sums are taken again around
+//       the mean, so the subtraction never loses more than six digits.
 //   T3: cut = k sigma in fp64; the fp64 test |x - mu| > cut is monotone in x on each side, so it
 //       equals two float compares x > t_hi, x < t_lo, with t_hi / t_lo found by evaluating the fp64
 //       predicate on the floats next to fl(mu +- cut).  The sweep is therefore exactly the fp64 test.
@@ -257,21 +258,31 @@ __device__ __forceinline__ void f32_window(float* x, int n, const TdF32Params& P
   const int wt = tl >> 5;
   int sel = 0;
   // ---------------------------------------------------------------- T2: statistics around the pivot
-  const double c = (double)x[0];
+  // A = sum (x - c), B = sum (x - c)^2, so mu = c + A/n and sigma^2 = B/n - (A/n)^2.  The subtraction cancels when
+  // the pivot is far from the mean in units of sigma (an RFI spike at x[0]; or the mean has moved after a huge
+  // sample was replaced): whenever sigma^2 < 1e-6 B/n -- more than six of the sixteen digits gone -- the sums are
+  // taken again around the current mean, where |A/n| is rounding noise.  Relative error of sigma^2 <= ~1e-10.
+  double c = (double)x[0];
   double A = 0.0, B = 0.0;
-  {
-    double A1 = 0.0, B1 = 0.0;
+  const double rn = 1.0 / (double)n;
+  auto sums = [&]() {
+    double A0 = 0.0, B0 = 0.0, A1 = 0.0, B1 = 0.0;
     int i = tl;
     for (; i + TT < n; i += 2 * TT) {
       const double d0 = (double)x[i] - c, d1 = (double)x[i + TT] - c;
-      A += d0; B = fma(d0, d0, B);
+      A0 += d0; B0 = fma(d0, d0, B0);
       A1 += d1; B1 = fma(d1, d1, B1);
     }
-    if (i < n) { const double d0 = (double)x[i] - c; A += d0; B = fma(d0, d0, B); }
-    A += A1; B += B1;
-  }
-  f32_team_sum2<kTW>(A, B, T, sel, wt, lane, team);
-  const double rn = 1.0 / (double)n;
+    if (i < n) { const double d0 = (double)x[i] - c; A0 += d0; B0 = fma(d0, d0, B0); }
+    A = A0 + A1; B = B0 + B1;
+    f32_team_sum2<kTW>(A, B, T, sel, wt, lane, team);
+  };
+  auto cancels = [&]() {                                 // team-uniform
+    const double am = A * rn, m2 = B * rn;
+    return m2 - am * am < 1e-6 * m2;
+  };
+  sums();
+  if (cancels()) { c += A * rn; sums(); }
   for (int it = 0; it < P.n_thr; ++it) {
     // ---------------------------------------------------------------- T3: bounds
     const double am = A * rn;
@@ -333,6 +344,11 @@ __device__ __forceinline__ void f32_window(float* x, int n, const TdF32Params& P
     if (it + 1 < P.n_thr) {
       f32_team_sum2<kTW>(dA, dB, T, sel, wt, lane, team);
       A += dA; B += dB;
+      if (cancels()) {                                   // the mean has left the pivot behind: sum again around it
+        f32_team_sync<kTW>(team);                        // every replacement of this iteration is visible
+        c += A * rn;
+        sums();
+      }
     }
     if (tl == 0 && P.counts) atomicAdd(&P.counts[it], (unsigned long long)cnt);
   }

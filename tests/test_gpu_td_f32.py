@@ -206,3 +206,24 @@ def test_iterations_equal_repeated_calls():
         y, f, c, _ = run_gpu(y, [3.0], policy="median", window=500)
         tot.append(int(c[0]))
     assert np.array_equal(a, y) and ca.tolist() == tot
+
+
+@pytest.mark.parametrize("policy", ["mean", "median"])
+@pytest.mark.parametrize("window", [0, 256, 1000])
+def test_huge_spike_at_the_first_sample_of_a_window(policy, window):
+    """An RFI spike of 1e6 .. 1e8 sigma that lands on a window's FIRST sample (a broadband impulse on a window
+    boundary does this to every channel at once).  The statistics must not be taken around that sample: with the
+    pivot 1e8 sigma away, sigma^2 = B/n - (A/n)^2 cancels completely in the iterations after the spike is replaced.
+    Three thresholds, so that two iterations run on statistics updated after the replacement."""
+    S = 12500
+    x = gauss((1, 24, S), seed=77)
+    W = S if window == 0 else window
+    amps = [1e6, 1e7, 1e8, -1e8, 3e7, 1e6]
+    for c in range(24):
+        a = np.float32(amps[c % len(amps)])
+        x[0, c, 0] = a                                   # first sample of the row = first sample of window 0
+        if W < S:
+            x[0, c, W * (1 + c % 5)] = a                 # first sample of another window
+            x[0, c, W * 7 + W // 2] = -a                 # and one in the middle of a window, for contrast
+    check(x, [4.0, 3.0, 3.0], policy=policy, window=window)
+    check(x, [5.0, 4.0, 3.0, 3.0], policy=policy, window=window, inplace=True)
