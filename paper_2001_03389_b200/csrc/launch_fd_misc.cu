@@ -23,6 +23,10 @@ int launch_fd_u8(const Call& c) {
     st = try_fd_u8_strip(c, true, 0, sms);
     if (st != RFIM_ERR_UNSUPPORTED) return st;
   }
+  if (c.variant == 17) {                              // the class-per-warp streaming kernel
+    st = try_fd_u8_quad(c, sms);
+    return st;
+  }
   if (c.variant == 0 || c.variant == 2 || c.variant == 16) {
     st = try_fd_u8_stream(c, sms);
     if (st != RFIM_ERR_UNSUPPORTED) return st;

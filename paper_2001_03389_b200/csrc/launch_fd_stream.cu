@@ -1,6 +1,7 @@
 // launch_fd_stream.cu -- geometry and launch of the streaming FDSC uint8 kernel (fd_u8_stream.cuh).
 #include "host.h"
 #include "fd_u8_stream.cuh"
+#include "fd_u8_quad.cuh"
 
 namespace rfim_host {
 
@@ -110,6 +111,75 @@ int launch_fd_stream(const Call& c, const StreamPlan& pl, int sms) {
     case 8: return launch_fd_stream_n<8>(c, pl, maps, P, sms);
     case 12: return launch_fd_stream_n<12>(c, pl, maps, P, sms);
     default: return launch_fd_stream_n<16>(c, pl, maps, P, sms);
+  }
+}
+
+// ---- one warp per alignment class (fd_u8_quad.cuh): one bin, channel counts of 128 * {4, 8, 12, 16}
+template <int NBQ>
+int launch_fd_quad_n(const Call& c, bool copy, const rfim::FdStreamMaps& maps, const rfim::FdStreamParams& P, int sms) {
+  void (*kernel)(const rfim::FdStreamMaps, const rfim::FdStreamParams) =
+      copy ? rfim::fd_u8_quad_kernel<NBQ, true> : rfim::fd_u8_quad_kernel<NBQ, false>;
+  const char* name = copy ? "fd_u8_quad_copy" : "fd_u8_quad";
+  const size_t smem = rfim::fd_quad_smem_bytes(NBQ);
+  int st = ensure_smem(kernel, smem);
+  if (st != RFIM_OK) return st;
+  int occ = 0;
+  if ((st = blocks_per_sm(kernel, rfim::kFqThreads, smem, occ)) != RFIM_OK) return st;
+  if (occ < 1) return RFIM_ERR_UNSUPPORTED;
+  int64_t grid = P.total_tiles;
+  if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  rfim::FdStreamParams Q = P;
+  bool owned = false;
+  if (c.workspace) {
+    Q.ticket = static_cast<unsigned int*>(c.workspace);
+  } else {
+    void* p = nullptr;
+    CUDA_TRY(cudaMallocAsync(&p, 256, c.stream));
+    Q.ticket = static_cast<unsigned int*>(p);
+    owned = true;
+  }
+  cudaError_t e = cudaMemsetAsync(Q.ticket, 0, sizeof(unsigned int), c.stream);
+  if (e != cudaSuccess) {
+    if (owned) cudaFreeAsync(Q.ticket, c.stream);
+    return cuda_fail(e, "cudaMemsetAsync(ticket)");
+  }
+  st = launch(name, kernel, dim3((unsigned)grid), dim3(rfim::kFqThreads), smem, c.stream, 0, maps, Q);
+  if (owned) {
+    e = cudaFreeAsync(Q.ticket, c.stream);
+    if (e != cudaSuccess && st == RFIM_OK) st = cuda_fail(e, "cudaFreeAsync(ticket)");
+  }
+  return st;
+}
+
+int try_fd_u8_quad(const Call& c, int sms) {
+  StreamPlan pl;
+  if (!plan_fd_u8_stream(c, pl) || pl.binned) return RFIM_ERR_UNSUPPORTED;   // same geometry limits, one bin only
+  rfim::FdStreamParams P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const uint8_t*>(c.data);
+  P.dst = static_cast<uint8_t*>(c.out);
+  P.stride = c.stride;
+  P.beams = c.beams; P.C = c.channels; P.S = c.samples;
+  P.n_thr = c.n_thr;
+  for (int i = 0; i < c.n_thr; ++i) P.p[i] = quantise(c.thr[i]);
+  P.flags = c.flags;
+  P.counts = c.counts;
+  P.tiles_per_beam = (c.samples + rfim::kFsCols - 1) / rfim::kFsCols;
+  P.total_tiles = (int64_t)P.tiles_per_beam * c.beams;
+  P.invC = (uint32_t)((((uint64_t)1 << 32) + (uint64_t)c.channels - 1) / (uint64_t)c.channels);
+  P.nb = c.channels;
+  ClassMaps cm;
+  if (!encode_class_maps(P.src, c.stride, c.samples, (int64_t)c.beams * c.channels, rfim::kFsPitchW * 4,
+                         rfim::kFsBoxRows, CU_TENSOR_MAP_L2_PROMOTION_NONE, cm))
+    return RFIM_ERR_UNSUPPORTED;
+  rfim::FdStreamMaps maps;
+  for (int k = 0; k < 4; ++k) { maps.src[k] = cm.m[k]; P.off[k] = cm.off[k]; }
+  switch (pl.nch) {                                    // channels / 128
+    case 4: return launch_fd_quad_n<4>(c, pl.copy, maps, P, sms);
+    case 8: return launch_fd_quad_n<8>(c, pl.copy, maps, P, sms);
+    case 12: return launch_fd_quad_n<12>(c, pl.copy, maps, P, sms);
+    default: return launch_fd_quad_n<16>(c, pl.copy, maps, P, sms);
   }
 }
 

@@ -32,7 +32,7 @@ def banded(shape, seed, block=32):
     return np.clip(x, 0, 255).astype(np.uint8)
 
 
-def check(x_np, ks, bin_size=0, inplace=False, pitch=None, want=None, base_shift=0):
+def check(x_np, ks, bin_size=0, inplace=False, pitch=None, want=None, base_shift=0, variant=STREAM):
     B, C, S = x_np.shape
     ref, rflags, rcounts = oracle.freq_sigma_cut(x_np, ks, bin_size=bin_size)
     P = pitch or S
@@ -44,7 +44,7 @@ def check(x_np, ks, bin_size=0, inplace=False, pitch=None, want=None, base_shift
     out = None if inplace else obuf[base_shift:base_shift + B * C * P].view(B, C, P)[:, :, :S]
     flags = torch.full((B, C, S), 7, dtype=torch.uint8, device=DEV)
     counts = torch.full((len(ks),), -1, dtype=torch.int64, device=DEV)
-    res = rfim.rfim_freq_sigma_cut(x, ks, out=out, bin_size=bin_size, flags=flags, counts=counts, variant=STREAM)
+    res = rfim.rfim_freq_sigma_cut(x, ks, out=out, bin_size=bin_size, flags=flags, counts=counts, variant=variant)
     torch.cuda.synchronize()
     name = rfim.rfim_last_variant()
     got = res.cpu().numpy()
