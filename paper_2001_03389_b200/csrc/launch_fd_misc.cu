@@ -12,22 +12,23 @@ int launch_fd_u8(const Call& c) {
   int st = sm_count(sms);
   if (st != RFIM_OK) return st;
 
-  // 0 = auto, 2 = any tuned kernel, 16 = the streaming kernel.  Auto order (measured on B200): one bin,
-  // out of place or a batch of fewer than about 200 beams -> the resident-tile strip kernel first (out of place it
-  // writes whole rows from shared memory; on short batches its tiles need no ticket ramp); everything else (large
-  // batches in place, bins) -> the streaming kernel first.
+  // 0 = auto, 2 = any tuned kernel, 16 = the streaming kernel, 17 = the class-per-warp streaming kernel.
+  // Auto order (measured on B200).  One bin: out of place, or a batch of fewer than about 200 beams,
+  // -> the resident-tile strip kernel first (out of place it writes whole rows from shared memory; on short batches
+  // its tiles need no ticket ramp); large batches in place -> the class-per-warp streaming kernel.  Bins -> the
+  // streaming kernel with per-bin sums.
   const bool one_bin = c.bin_size == c.channels;
+  const bool tuned = c.variant == 0 || c.variant == 2;
   const int64_t tiles = (int64_t)c.beams * ((c.samples + 127) / 128);
-  const bool strip_first = (c.variant == 0 || c.variant == 2) && one_bin && (c.out != c.data || tiles < 20000);
-  if (strip_first) {
+  if (tuned && one_bin && (c.out != c.data || tiles < 20000)) {
     st = try_fd_u8_strip(c, true, 0, sms);
     if (st != RFIM_ERR_UNSUPPORTED) return st;
   }
-  if (c.variant == 17) {                              // the class-per-warp streaming kernel
+  if (tuned || c.variant == 17) {
     st = try_fd_u8_quad(c, sms);
-    return st;
+    if (st != RFIM_ERR_UNSUPPORTED || c.variant == 17) return st;
   }
-  if (c.variant == 0 || c.variant == 2 || c.variant == 16) {
+  if (tuned || c.variant == 16) {
     st = try_fd_u8_stream(c, sms);
     if (st != RFIM_ERR_UNSUPPORTED) return st;
     if (c.variant == 16) return RFIM_ERR_UNSUPPORTED;

@@ -1,6 +1,7 @@
 // launch_td_f32.cu -- geometry and launch of the TDSC float32 kernel (td_f32.cuh).
 #include "host.h"
 #include "td_f32.cuh"
+#include "td_f32_fast.cuh"
 
 namespace rfim_host {
 
@@ -20,6 +21,49 @@ int launch_td_f32_t(const Call& c, rfim::TdF32Params& P, bool stage, int sms, co
   return launch(name, kernel, dim3((unsigned)grid), dim3(rfim::kF32Threads), smem, c.stream, 0, P);
 }
 
+// ---- the tuned kernel (td_f32_fast.cuh): whole rows staged in shared memory, windows that are multiples of 4 samples
+// (or the whole row), a team of G lanes per window
+template <int G>
+int launch_td_f32_fast_g(const Call& c, const rfim::TdF32Params& P, int sms, const char* name) {
+  const size_t smem = rfim::f32_fast_smem_bytes(P.S, G);
+  void (*kernel)(const rfim::TdF32Params) = rfim::td_f32_fast_kernel<G>;
+  int st = ensure_smem(kernel, smem);
+  if (st != RFIM_OK) return st;
+  int occ = 0;
+  if ((st = blocks_per_sm(kernel, rfim::kF32FastThreads, smem, occ)) != RFIM_OK) return st;
+  if (occ < 1) return RFIM_ERR_UNSUPPORTED;
+  int64_t grid = P.rows;
+  if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  return launch(name, kernel, dim3((unsigned)grid), dim3(rfim::kF32FastThreads), smem, c.stream, 0, P);
+}
+int try_td_f32_fast(const Call& c, const rfim::TdF32Params& P, int sms) {
+  const uintptr_t a = reinterpret_cast<uintptr_t>(c.data) | reinterpret_cast<uintptr_t>(c.out);
+  if ((a & 15) != 0 || (c.stride % 4 != 0 && P.rows != 1) || c.samples % 4 != 0) return RFIM_ERR_UNSUPPORTED;
+  const int W = c.window;                               // already clamped to samples
+  if (W != c.samples && W % 4 != 0) return RFIM_ERR_UNSUPPORTED;
+  if (W > 32768) return RFIM_ERR_UNSUPPORTED;
+  const int nwin = (c.samples + W - 1) / W;
+  // the smallest team that leaves a lane at most 16 quads (W = 256 -> 4 lanes, 1024 -> 16, 4096 -> 64, longer -> the
+  // CTA): short windows keep their scalar chain (square root, bounds, reductions) on few lanes, long ones spread
+  int best = 0;
+  for (int G = 4; G <= 256; G *= 4) {
+    if (W > 64 * G && G != 256) continue;
+    if (W > 128 * G) continue;                          // at most 32 quads per lane (bit mask of flagged quads)
+    if (rfim::f32_fast_smem_bytes(c.samples, G) > (size_t)kMaxSmem) continue;
+    best = G;
+    break;
+  }
+  (void)nwin;
+  switch (best) {
+    case 4: return launch_td_f32_fast_g<4>(c, P, sms, "td_f32_fast_g4");
+    case 16: return launch_td_f32_fast_g<16>(c, P, sms, "td_f32_fast_g16");
+    case 64: return launch_td_f32_fast_g<64>(c, P, sms, "td_f32_fast_g64");
+    case 256: return launch_td_f32_fast_g<256>(c, P, sms, "td_f32_fast_g256");
+    default: return RFIM_ERR_UNSUPPORTED;
+  }
+}
+
 int launch_td_f32(const Call& c) {
   rfim::TdF32Params P;
   memset(&P, 0, sizeof(P));
@@ -37,6 +81,11 @@ int launch_td_f32(const Call& c) {
   int sms = 0;
   int st = sm_count(sms);
   if (st != RFIM_OK) return st;
+  // variant 0 / 2: the tuned kernel when the request fits it; 3 / 4: the segment kernel below even then (testing)
+  if ((c.variant == 0 || c.variant == 2) && c.reserved_team == 0) {
+    st = try_td_f32_fast(c, P, sms);
+    if (st != RFIM_ERR_UNSUPPORTED) return st;
+  }
   // segment = run of whole windows staged in shared memory: the whole row when it fits beside the team
   // scratch with three CTAs per SM, else the whole row alone, else as many windows as fit
   const int overhead = 8 * (int)sizeof(rfim::F32Team) + 16;

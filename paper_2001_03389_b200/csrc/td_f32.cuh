@@ -343,8 +343,11 @@ __device__ __forceinline__ void f32_window(float* x, int n, const TdF32Params& P
     }
     if (it + 1 < P.n_thr) {
       f32_team_sum2<kTW>(dA, dB, T, sel, wt, lane, team);
+      const double B_before = B;
       A += dA; B += dB;
-      if (cancels()) {                                   // the mean has left the pivot behind: sum again around it
+      // sum again around the current mean when the update cannot be trusted: the mean has left the pivot behind, or
+      // the replaced samples carried nearly all of B (a 1e8 sigma spike: B was 1e16 + the rest, in 53 bits)
+      if (cancels() || B < 1e-6 * B_before) {
         f32_team_sync<kTW>(team);                        // every replacement of this iteration is visible
         c += A * rn;
         sums();

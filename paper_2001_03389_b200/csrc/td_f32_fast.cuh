@@ -1,0 +1,418 @@
+// td_f32_fast.cuh -- time-domain sigma cut (TDSC, Fig. 2) for float32 dynamic spectra with statistics
+// windows and mean / lower-median replacement (BASELINE.json configs[4]): the tuned kernel for rows
+// that fit shared memory and windows that are multiples of 4 samples (td_f32.cuh keeps every other request).
+//
+// What the ncu captures of td_f32_kernel showed (profiles/r2a_f32_*): 110 - 130 thread instructions per sample, i.e.
+// the kernel was bound by its own instruction count -- scalar strided loops (8 instructions per element and pass),
+// about ten passes per window for the median (a 258-bin histogram with shared-memory atomics, a compaction pass, a
+// ranking), and for short windows a per-window scalar chain (fp64 square root, bounds, reductions) executed by all
+// 32 lanes of a warp for 8 elements each.  This kernel does the same arithmetic with a third of the instructions:
+//   T1  one CTA of 256 threads stages a whole row by one 1-D TMA bulk copy (as before).
+//   --  a window is owned by a TEAM of G lanes, G in {4, 16, 64, 256} chosen on the host so that a lane holds at most
+//       32 quads (16 for the config-5 windows) and all 256 threads have work: W = 256 -> 4 lanes (8 windows per
+//       warp side by side, each with its own scalar chain), W = 1024 -> 16, the whole row -> the CTA.  Teams of a
+//       warp diverge freely: every shuffle carries the team's own lane mask.
+//   T2  one pass of 128-bit shared-memory loads; fp64 sums around a pivot, re-taken around the mean whenever the
+//       subtraction sigma^2 = B/n - (A/n)^2 would lose more than six digits (td_f32.cuh has the argument).
+//   T3  cut = k sigma in fp64 -> two float bounds that reproduce the fp64 test exactly (f32_bounds).
+//   T4  detection pass: FMNMX over a quad, two compares per quad, a bit per flagged quad; the replacement pass visits
+//       the flagged quads only.
+//   T2m lower median by BRACKETING: counting passes with two pivots (from mu, sigma, then by interpolation) shrink
+//       the value interval that holds rank (n-1)/2 to at most 32 elements, which are gathered (as 16-bit indices)
+//       and ranked.  And it is taken at most ONCE per window: replacing samples by the lower median m never changes
+//       the lower median -- with L samples < m and E samples = m (L <= rank < L + E), moving l samples from below
+//       and u from above onto m gives L - l <= rank < L + E + u -- so every later iteration's snapshot median is m.
+//   T5  statistics of the next iteration from the fp64 deltas of the replaced samples.   T6  one TMA bulk store.
+#pragma once
+
+#include "common.cuh"
+#include "td_f32.cuh"   // TdF32Params, f32_bounds, f32_key
+
+namespace rfim {
+
+constexpr int kF32FastThreads = 256;
+constexpr int kF32FastListCap = 32;    // capacity of a team's gather list (f32f_cap<G>() <= this)
+
+// scratch of one team in shared memory
+struct __align__(8) F32FastTeam {
+  uint16_t list[kF32FastListCap];   // gathered candidates: element indices inside the window
+  int ln;                           // gather cursor
+  float result;
+};
+// exchange area of the teams that span several warps (G >= 64): at most 4 teams x 8 warps
+struct __align__(16) F32FastXchg {
+  double red[2][8][2];
+  uint32_t redu[2][8];
+};
+__host__ __device__ constexpr int f32_fast_teams(int G) { return kF32FastThreads / G; }
+__host__ __device__ inline size_t f32_fast_smem_bytes(int S, int G) {
+  size_t b = ((size_t)S * 4 + 15) & ~(size_t)15;
+  b += (size_t)f32_fast_teams(G) * sizeof(F32FastTeam);
+  if (G > 32) b = ((b + 15) & ~(size_t)15) + (size_t)f32_fast_teams(G) * sizeof(F32FastXchg);
+  return b + 16;
+}
+
+template <int G>
+struct F32FastCtx {
+  F32FastTeam* T;
+  F32FastXchg* X;     // G > 32 only
+  uint32_t tmask;     // lanes of this team inside its warp (G <= 32), else FULL
+  int j;              // lane index inside the team
+  int team;           // team index inside the CTA
+  int lane, wt;       // lane inside the warp, warp inside the team
+  int sel;            // exchange buffer
+};
+
+template <int G>
+__device__ __forceinline__ void f32f_sync(const F32FastCtx<G>& c) {
+  if (G <= 32) __syncwarp(c.tmask);
+  else if (G == kF32FastThreads) __syncthreads();
+  else asm volatile("bar.sync %0, %1;" ::"r"(c.team + 1), "n"(G) : "memory");
+}
+template <int G>
+__device__ __forceinline__ void f32f_sum2(double& a, double& b, F32FastCtx<G>& c) {
+  constexpr int W = G < 32 ? G : 32;
+#pragma unroll
+  for (int o = W / 2; o > 0; o >>= 1) {
+    a += __shfl_xor_sync(c.tmask, a, o);
+    b += __shfl_xor_sync(c.tmask, b, o);
+  }
+  if (G > 32) {
+    if (c.lane == 0) { c.X->red[c.sel][c.wt][0] = a; c.X->red[c.sel][c.wt][1] = b; }
+    f32f_sync<G>(c);
+    a = 0.0; b = 0.0;
+#pragma unroll
+    for (int w = 0; w < G / 32; ++w) { a += c.X->red[c.sel][w][0]; b += c.X->red[c.sel][w][1]; }
+    c.sel ^= 1;
+  }
+}
+template <int G>
+__device__ __forceinline__ uint32_t f32f_sum_u32(uint32_t a, F32FastCtx<G>& c) {
+  constexpr int W = G < 32 ? G : 32;
+  if (W == 32) {
+    a = __reduce_add_sync(FULL, a);
+  } else {
+#pragma unroll
+    for (int o = W / 2; o > 0; o >>= 1) a += __shfl_xor_sync(c.tmask, a, o);
+  }
+  if (G > 32) {
+    if (c.lane == 0) c.X->redu[c.sel][c.wt] = a;
+    f32f_sync<G>(c);
+    a = 0;
+#pragma unroll
+    for (int w = 0; w < G / 32; ++w) a += c.X->redu[c.sel][w];
+    c.sel ^= 1;
+  }
+  return a;
+}
+
+// A lane's quads of a window of nq quads: j, j + G, ..., j + G (T - 1).  They are visited in the rotated order t0,
+// t0 + 1, ..., T - 1, 0, ..., t0 - 1, so that the teams sharing a quarter-warp read different bank groups (G < 8
+// only).  body(quad index, t).
+struct F32Quads { int T, t0; };
+template <int G, typename F>
+__device__ __forceinline__ void f32f_each_quad(const F32Quads& q, int j, F&& body) {
+  if (G < 8) {
+#pragma unroll 2
+    for (int t = q.t0; t < q.T; ++t) body(j + G * t, t);
+    for (int t = 0; t < q.t0; ++t) body(j + G * t, t);
+  } else {
+#pragma unroll 2
+    for (int t = 0; t < q.T; ++t) body(j + G * t, t);
+  }
+}
+// elements a team gathers and ranks at the end of the median search: the ranking costs m^2 / G compares per lane
+template <int G>
+__host__ __device__ constexpr int f32f_cap() { return G <= 4 ? 12 : (G <= 16 ? 16 : 32); }
+
+// T2m: lower median (rank (n-1)/2 of the ascending values) of the window x4[0 .. n/4), by the whole team; every
+// lane returns it.  mu / sigma (floats) only guide the first pivots.  The values are only read.
+template <int G>
+__device__ float f32f_median(const float4* x4, int n, const F32Quads& Q, float muf, float sigf, F32FastCtx<G>& c) {
+  const float* x = reinterpret_cast<const float*>(x4);
+  const uint32_t rho = (uint32_t)(n - 1) >> 1;
+  const float inf = __int_as_float(0x7f800000);
+  // invariant: #{v <= a} = ca <= rho < cb = #{v <= b}; the answer is the (rho - ca)-th smallest value in (a, b]
+  float a = -inf, b = inf;
+  uint32_t ca = 0, cb = (uint32_t)n;
+  // first pivots: the median of n Gaussian draws is within 1.25 sigma / sqrt(n) (one standard deviation) of mu
+  float R = 3.2f * sigf * rsqrtf((float)n);
+  float p1 = muf - R, p2 = muf + R;
+  for (int pass = 0; pass < 64 && cb - ca > (uint32_t)f32f_cap<G>(); ++pass) {
+    if (!(p1 > a)) p1 = a;                               // keep the pivots inside the bracket (also rejects NaN)
+    if (!(p2 < b)) p2 = b;
+    if (!(p1 <= p2)) p1 = p2;
+    uint32_t c1 = 0, c12 = 0;                            // #{v <= p1}, #{v <= p1} + #{v <= p2}
+    f32f_each_quad<G>(Q, c.j, [&](int qi, int) {
+      const float4 v = x4[qi];
+      const uint32_t a0 = v.x <= p1, a1 = v.y <= p1, a2 = v.z <= p1, a3 = v.w <= p1;
+      const uint32_t b0 = v.x <= p2, b1 = v.y <= p2, b2 = v.z <= p2, b3 = v.w <= p2;
+      c1 += a0 + a1; c1 += a2 + a3;
+      c12 += b0 + b1; c12 += b2 + b3;
+    });
+    // one reduction for both counts: n <= 2^15 in this kernel (the host checks), so each fits 16 bits
+    const uint32_t packed = f32f_sum_u32<G>(c1 | (c12 << 16), c);
+    c1 = packed & 0xffffu;
+    const uint32_t c2 = packed >> 16;
+    if (rho < c1) { b = p1; cb = c1; }
+    else if (rho < c2) { a = p1; ca = c1; b = p2; cb = c2; }
+    else { a = p2; ca = c2; }
+    const uint32_t m = cb - ca;
+    if (m <= (uint32_t)f32f_cap<G>()) break;
+    // next pivots
+    if (a > -inf && b < inf && b > a) {
+      // interpolate the rank inside (a, b] and step aside by a margin of a few binomial standard deviations
+      const float w = b - a;
+      if (!(w <= 3.0e38f)) break;                        // (unreachable for |x| < 1e18: key bisection below)
+      const float f = ((float)(rho - ca) + 0.5f) / (float)m;
+      const float dev = (2.0f * sqrtf(f * (1.0f - f) * (float)m) + 1.0f) / (float)m;
+      p1 = a + w * fmaxf(f - dev, 0.0f);
+      p2 = a + w * fminf(f + dev, 1.0f);
+      if (!(p1 > a)) p1 = f32_next_up(a);                // the float grid is exhausted towards a
+      if (!(p1 < b)) return b;                           // a and b are neighbouring floats: every value in (a, b] is b
+      if (!(p2 < b)) p2 = f32_next_down(b);
+      if (!(p2 >= p1)) p2 = p1;
+    } else if (b == inf && a == -inf) {                  // (both pivots collapsed: cannot happen, but stay finite)
+      p1 = muf - 2.0f * R; p2 = muf + 2.0f * R; R *= 2.0f;
+    } else if (b == inf) {                               // everything seen so far lies below the rank: go up
+      R *= 4.0f;
+      p1 = a + R; p2 = a + 4.0f * R;
+      if (!(p1 > a)) { p1 = 3.402823466e38f; p2 = 3.402823466e38f; }
+      if (!(p2 < inf)) p2 = 3.402823466e38f;
+    } else {                                             // a == -inf: go down
+      R *= 4.0f;
+      p2 = b - R; p1 = b - 4.0f * R;
+      if (!(p2 < b)) { p1 = -3.402823466e38f; p2 = -3.402823466e38f; }
+      if (!(p1 > -inf)) p1 = -3.402823466e38f;
+    }
+  }
+  const uint32_t m = cb - ca;
+  if (m > (uint32_t)f32f_cap<G>()) {
+    // last resort (64 passes did not shrink the bracket: a pathological value distribution): bisection on the
+    // order-preserving integer keys, 32 counting passes, always terminates
+    uint32_t klo = 0u, khi = 0xffffffffu;
+    while (klo < khi) {
+      const uint32_t mid = klo + ((khi - klo) >> 1);
+      uint32_t cnt = 0;
+      f32f_each_quad<G>(Q, c.j, [&](int qi, int) {
+        const float4 v = x4[qi];
+        cnt += (f32_key(v.x) <= mid) + (f32_key(v.y) <= mid) + (f32_key(v.z) <= mid) + (f32_key(v.w) <= mid);
+      });
+      cnt = f32f_sum_u32<G>(cnt, c);
+      if (cnt > rho) khi = mid; else klo = mid + 1;
+    }
+    const uint32_t bits = (klo & 0x80000000u) ? (klo & 0x7fffffffu) : ~klo;
+    return __int_as_float((int)bits);
+  }
+  // gather the (at most 32) elements of (a, b] as indices, then rank them: the one with rank rho - ca is the median
+  if (c.j == 0) c.T->ln = 0;
+  f32f_sync<G>(c);
+  f32f_each_quad<G>(Q, c.j, [&](int qi, int) {
+    const float4 v = x4[qi];
+    // a quad holds a value of (a, b] only if ... cheap necessary test first: most quads hold none
+    const bool in0 = v.x > a && v.x <= b, in1 = v.y > a && v.y <= b, in2 = v.z > a && v.z <= b, in3 = v.w > a && v.w <= b;
+    if (in0 | in1 | in2 | in3) {
+      if (in0) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi);
+      if (in1) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 1);
+      if (in2) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 2);
+      if (in3) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 3);
+    }
+  });
+  f32f_sync<G>(c);
+  const uint32_t want = rho - ca;
+  for (uint32_t i = (uint32_t)c.j; i < m; i += G) {
+    const uint32_t ii = c.T->list[i];
+    const float e = x[ii];
+    uint32_t rank = 0;
+    for (uint32_t k = 0; k < m; ++k) {
+      const uint32_t kk = c.T->list[k];
+      const float o = x[kk];
+      rank += (o < e) || (o == e && kk < ii);
+    }
+    if (rank == want) c.T->result = e;
+  }
+  f32f_sync<G>(c);
+  const float r = c.T->result;
+  f32f_sync<G>(c);                                       // nobody reads the scratch after this point
+  return r;
+}
+
+// One window, all thresholds, by one team.  x4 points at the window in shared memory, n is a multiple of 4.
+template <int G>
+__device__ __forceinline__ void f32f_window(float4* x4, int n, const TdF32Params& P, uint8_t* flags, int team_in_warp,
+                                            F32FastCtx<G>& c) {
+  const int nq = n >> 2;
+  F32Quads Q;
+  Q.T = nq > c.j ? (nq - c.j + G - 1) / G : 0;
+  Q.t0 = 0;
+  if (G < 8 && Q.T > 0) Q.t0 = (team_in_warp & (8 / G - 1)) % Q.T;
+  const float* xs = reinterpret_cast<const float*>(x4);
+  // ---------------------------------------------------------------- T2: statistics around the pivot
+  double piv = (double)xs[0];
+  double A = 0.0, B = 0.0;
+  const double rn = 1.0 / (double)n;
+  auto sums = [&]() {
+    double A0 = 0.0, B0 = 0.0, A1 = 0.0, B1 = 0.0;
+    f32f_each_quad<G>(Q, c.j, [&](int qi, int) {
+      const float4 v = x4[qi];
+      const double d0 = (double)v.x - piv, d1 = (double)v.y - piv, d2 = (double)v.z - piv, d3 = (double)v.w - piv;
+      A0 += d0; B0 = fma(d0, d0, B0);
+      A1 += d1; B1 = fma(d1, d1, B1);
+      A0 += d2; B0 = fma(d2, d2, B0);
+      A1 += d3; B1 = fma(d3, d3, B1);
+    });
+    A = A0 + A1; B = B0 + B1;
+    f32f_sum2<G>(A, B, c);
+  };
+  auto cancels = [&]() {                                 // team-uniform
+    const double am = A * rn, m2 = B * rn;
+    return m2 - am * am < 1e-6 * m2;
+  };
+  sums();
+  if (cancels()) { piv += A * rn; sums(); }
+
+  bool have_median = false;
+  float median = 0.0f;
+  for (int it = 0; it < P.n_thr; ++it) {
+    // ---------------------------------------------------------------- T3: bounds
+    const double am = A * rn;
+    const double mu = piv + am;
+    double var = B * rn - am * am;
+    if (!(var > 0.0)) var = 0.0;
+    const double sigma = sqrt(var);
+    const double cut = P.k[it] * sigma;
+    float t_lo, t_hi;
+    f32_bounds(mu, cut, t_lo, t_hi);
+    // ---------------------------------------------------------------- T4: detect (a bit per flagged quad)
+    uint32_t fm = 0;                                     // bit t <=> the lane's quad j + G t holds a flagged sample
+    f32f_each_quad<G>(Q, c.j, [&](int qi, int t) {
+      const float4 v = x4[qi];
+      const float lo = fminf(fminf(v.x, v.y), fminf(v.z, v.w)), hi = fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w));
+      if (hi > t_hi || lo < t_lo) fm |= 1u << t;
+    });
+    uint32_t cnt = 0;
+    if (fm) {
+      uint32_t f2 = fm;
+      while (f2) {
+        const int t = __ffs(f2) - 1;
+        f2 &= f2 - 1;
+        const float4 v = x4[c.j + G * t];
+        cnt += (v.x > t_hi || v.x < t_lo) + (v.y > t_hi || v.y < t_lo) + (v.z > t_hi || v.z < t_lo) +
+               (v.w > t_hi || v.w < t_lo);
+      }
+    }
+    cnt = f32f_sum_u32<G>(cnt, c);
+    if (cnt == 0) continue;                              // team-uniform
+    // ---------------------------------------------------------------- T2m / replacement value
+    float r;
+    if (P.policy == 0) {
+      r = (float)mu;
+    } else {
+      if (!have_median) {
+        median = f32f_median<G>(x4, n, Q, (float)mu, (float)sigma, c);
+        have_median = true;
+      }
+      r = median;
+    }
+    // ---------------------------------------------------------------- T4: replace, T5: deltas
+    double dA = 0.0, dB = 0.0;
+    const double dr = (double)r - piv;
+    while (fm) {
+      const int t = __ffs(fm) - 1;
+      fm &= fm - 1;
+      const int qi = c.j + G * t;
+      float4 v = x4[qi];
+      float* pv = reinterpret_cast<float*>(&v);
+#pragma unroll
+      for (int u = 0; u < 4; ++u) {
+        const float e = pv[u];
+        if (e > t_hi || e < t_lo) {
+          const double d = (double)e - piv;
+          dA += dr - d; dB += dr * dr - d * d;
+          pv[u] = r;
+          if (flags) flags[4 * qi + u] = 1;
+        }
+      }
+      x4[qi] = v;
+    }
+    if (it + 1 < P.n_thr) {
+      f32f_sum2<G>(dA, dB, c);                           // (for G <= 32 the shuffles also order the team's writes)
+      const double B_before = B;
+      A += dA; B += dB;
+      // sum again around the current mean when the update cannot be trusted: the mean has left the pivot behind, or
+      // the replaced samples carried nearly all of B (a 1e8 sigma spike: B was 1e16 + the rest, in 53 bits)
+      if (cancels() || B < 1e-6 * B_before) {
+        f32f_sync<G>(c);
+        piv += A * rn;
+        sums();
+      }
+    }
+    if (c.j == 0 && P.counts) atomicAdd(&P.counts[it], (unsigned long long)cnt);
+  }
+}
+
+// dynamic shared memory: [row: S floats][teams x F32FastTeam][G > 32: teams x F32FastXchg][mbarrier]
+template <int G>
+__global__ void __launch_bounds__(kF32FastThreads, 4) td_f32_fast_kernel(const TdF32Params P) {
+  extern __shared__ __align__(128) uint8_t smem[];
+  constexpr int NT = kF32FastThreads / G;
+  const size_t row_bytes = ((size_t)P.S * 4 + 15) & ~(size_t)15;
+  float* slot = reinterpret_cast<float*>(smem);
+  F32FastTeam* teams = reinterpret_cast<F32FastTeam*>(smem + row_bytes);
+  size_t off = row_bytes + (size_t)NT * sizeof(F32FastTeam);
+  F32FastXchg* xchg = nullptr;
+  if (G > 32) {
+    off = (off + 15) & ~(size_t)15;
+    xchg = reinterpret_cast<F32FastXchg*>(smem + off);
+    off += (size_t)NT * sizeof(F32FastXchg);
+  }
+  uint64_t* bar = reinterpret_cast<uint64_t*>(smem + ((off + 7) & ~(size_t)7));
+  const int tid = threadIdx.x, lane = tid & 31;
+  F32FastCtx<G> c;
+  c.team = tid / G;
+  c.j = tid % G;
+  c.lane = lane;
+  c.wt = (tid % G) >> 5;
+  c.sel = 0;
+  c.T = teams + c.team;
+  c.X = G > 32 ? xchg + c.team : nullptr;
+  c.tmask = G >= 32 ? FULL : (((1u << (G & 31)) - 1u) << (lane & ~(G - 1)));
+  const int team_in_warp = G >= 32 ? 0 : (lane / G);
+  if (tid == 0) {
+    mbar_init(bar, 1);
+    fence_mbar_init();
+  }
+  __syncthreads();
+  uint32_t phase = 0;
+  const int nwin = (P.S + P.window - 1) / P.window;
+  for (int64_t row = blockIdx.x; row < P.rows; row += gridDim.x) {
+    const float* g = P.src + row * P.stride;
+    float* go = P.dst + row * P.stride;
+    // ---------------------------------------------------------------- T1: load (S is a multiple of 4)
+    if (tid == 0) {
+      mbar_arrive_expect_tx(bar, (uint32_t)P.S * 4u);
+      bulk_load(slot, g, (uint32_t)P.S * 4u, bar);
+    }
+    mbar_wait(bar, phase);
+    phase ^= 1;
+    // ---------------------------------------------------------------- T2..T5: windows of the row
+    uint8_t* fl = P.flags ? P.flags + row * P.S : nullptr;
+    for (int w = c.team; w < nwin; w += NT) {
+      const int w0 = w * P.window;
+      f32f_window<G>(reinterpret_cast<float4*>(slot + w0), min(P.window, P.S - w0), P, fl ? fl + w0 : nullptr,
+                     team_in_warp, c);
+    }
+    // ---------------------------------------------------------------- T6: store
+    fence_proxy_async_smem();
+    __syncthreads();
+    if (tid == 0) {
+      bulk_store(go, slot, (uint32_t)P.S * 4u);
+      bulk_commit();
+      bulk_wait_read<0>();
+    }
+    __syncthreads();
+  }
+  if (tid == 0) bulk_wait_all<0>();
+}
+
+}  // namespace rfim

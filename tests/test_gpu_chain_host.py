@@ -37,7 +37,7 @@ def test_chain_config4_slice(inplace):
     counts = torch.full((5,), -1, dtype=torch.int64, device=DEV)
     res = rfim.rfim_time_freq_sigma_cut(xd, cfg["thresholds"], cfg["freq_thresholds"], out=out, flags=flags, counts=counts)
     torch.cuda.synchronize()
-    assert rfim.rfim_last_variant() in ("fd_u8_stream", "fd_u8_strip1")
+    assert rfim.rfim_last_variant() in ("fd_u8_quad", "fd_u8_stream", "fd_u8_strip1")
     assert np.array_equal(res.cpu().numpy(), ref)
     assert np.array_equal(flags.cpu().numpy(), rflags)
     assert counts.cpu().tolist() == rcounts and min(rcounts) > 0

@@ -87,10 +87,10 @@ def test_config3_arts_like_all_beams():
     synth.fill_device(cfg, x)
     x_np = x.cpu().numpy()
     name, counts = check(x_np, cfg["thresholds"], inplace=True)      # auto: the strip kernel on a 12-beam batch
-    assert name in ("fd_u8_strip1", "fd_u8_stream")
+    assert name in ("fd_u8_strip1", "fd_u8_quad", "fd_u8_stream")
     assert all(int(c) > 0 for c in counts)
     name, _ = check(x_np[:3], cfg["thresholds"])                      # auto, out of place
-    assert name in ("fd_u8_strip1", "fd_u8_stream_copy")
+    assert name in ("fd_u8_strip1", "fd_u8_quad_copy", "fd_u8_stream_copy")
     name, _ = check(x_np[:3], cfg["thresholds"], inplace=True, variant=STREAM)
     assert name == "fd_u8_stream"
     name, _ = check(x_np[:2], cfg["thresholds"], variant=STREAM)      # out of place: copy + repair

@@ -44,7 +44,7 @@ def test_config4_full_size_chain_sampled_beams():
     counts = torch.zeros(5, dtype=torch.int64, device=DEV)
     rfim.rfim_time_freq_sigma_cut(x, cfg["thresholds"], cfg["freq_thresholds"], out=y, counts=counts)
     torch.cuda.synchronize()
-    assert rfim.rfim_last_variant() == "fd_u8_stream"
+    assert rfim.rfim_last_variant() == "fd_u8_quad"
     xs = torch.stack([x[b] for b in SAMPLE_BEAMS]).cpu().numpy()
     ys = torch.stack([y[b] for b in SAMPLE_BEAMS]).cpu().numpy()
     # the generator twins agree at these offsets too (the host twin feeds the oracle elsewhere)

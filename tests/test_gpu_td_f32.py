@@ -134,7 +134,7 @@ def test_padded_pitch_and_global_variant(variant, pitch, inplace):
     x = gauss((2, 7, 1000), seed=pitch)
     x[0, 2, 100:110] += 12.0
     name, _ = check(x, [4.0, 3.0], policy="median", window=256, variant=variant, pitch=pitch, inplace=inplace)
-    assert name.startswith("td_f32_global" if variant == rfim.VARIANT_GENERIC else "td_f32_staged")
+    assert name.startswith("td_f32_global" if variant == rfim.VARIANT_GENERIC else ("td_f32_staged", "td_f32_fast"))
 
 
 @pytest.mark.parametrize("window,expect", [(0, "td_f32_global_w8"), (1024, "td_f32_staged_w1"),
@@ -227,3 +227,30 @@ def test_huge_spike_at_the_first_sample_of_a_window(policy, window):
             x[0, c, W * 7 + W // 2] = -a                 # and one in the middle of a window, for contrast
     check(x, [4.0, 3.0, 3.0], policy=policy, window=window)
     check(x, [5.0, 4.0, 3.0, 3.0], policy=policy, window=window, inplace=True)
+
+
+@pytest.mark.parametrize("policy", ["mean", "median"])
+@pytest.mark.parametrize("window", [0, 256, 1000])
+def test_segment_kernel_forced(policy, window):
+    """The tuned kernel (td_f32_fast.cuh) takes these requests in auto mode; variant 3 keeps the segment kernel
+    (td_f32.cuh), which still serves rows longer than shared memory, windows that are not multiples of 4 samples
+    and unaligned rows, under test on the same inputs."""
+    cfg = synth.config(5, beams=1, channels=32)
+    x = synth.fill_host(cfg)
+    name, _ = check(x, cfg["thresholds"], policy=policy, window=window, variant=rfim.VARIANT_STAGED_1W)
+    assert name.startswith("td_f32_staged")
+    name, _ = check(x, cfg["thresholds"], policy=policy, window=window)
+    assert name.startswith("td_f32_fast")
+
+
+@pytest.mark.parametrize("window,team", [(4, 4), (64, 4), (256, 4), (260, 16), (1024, 16), (1028, 64), (4096, 64),
+                                         (4100, 256), (12500, 256)])
+def test_fast_kernel_team_sizes(window, team):
+    """Every team size of the tuned kernel, windows at the edges of each range, a ragged last window."""
+    x = gauss((1, 12, 12500), seed=window)
+    x[0, 1, 5000:5040] += 9.0
+    x[0, 2, ::1250] = 30.0
+    x[0, 3, 12499] = -1e4
+    for policy in ("mean", "median"):
+        name, _ = check(x, [4.0, 3.0, 3.0], policy=policy, window=window)
+        assert name == f"td_f32_fast_g{team}"
