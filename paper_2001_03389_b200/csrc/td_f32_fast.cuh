@@ -106,6 +106,14 @@ __device__ __forceinline__ uint32_t f32f_sum_u32(uint32_t a, F32FastCtx<G>& c) {
   return a;
 }
 
+// 0xFFFFFFFF if v <= p else 0 (one FSET; false for NaN).  Counting with these masks -- c -= m0 + m1 -- costs 1.5
+// instructions per compare; `c += (v <= p)` compiles to a compare, an add and a predicated move on one dependent chain.
+__device__ __forceinline__ uint32_t f32f_le_mask(float v, float p) {
+  uint32_t m;
+  asm("set.le.u32.f32 %0, %1, %2;" : "=r"(m) : "f"(v), "f"(p));
+  return m;
+}
+
 // A lane's quads of a window of nq quads: j, j + G, ..., j + G (T - 1).  They are visited in the rotated order t0,
 // t0 + 1, ..., T - 1, 0, ..., t0 - 1, so that the teams sharing a quarter-warp read different bank groups (G < 8
 // only).  body(quad index, t).
@@ -125,99 +133,133 @@ __device__ __forceinline__ void f32f_each_quad(const F32Quads& q, int j, F&& bod
 template <int G>
 __host__ __device__ constexpr int f32f_cap() { return G <= 4 ? 12 : (G <= 16 ? 16 : 32); }
 
-// T2m: lower median (rank (n-1)/2 of the ascending values) of the window x4[0 .. n/4), by the whole team; every
-// lane returns it.  mu / sigma (floats) only guide the first pivots.  The values are only read.
+// Teams narrower than a warp run side by side in one warp.  Their heavy loops must stay CONVERGED (a warp that
+// splits into its teams executes every loop once per team), so the control flow around them is warp-uniform: every
+// lane of the warp takes part, a team that has nothing to do makes zero trips, and loop conditions are votes.
 template <int G>
-__device__ float f32f_median(const float4* x4, int n, const F32Quads& Q, float muf, float sigf, F32FastCtx<G>& c) {
+__device__ __forceinline__ bool f32f_any(bool p) {
+  return G < 32 ? __any_sync(FULL, p) : p;             // G >= 32: the team owns its warps, p is team-uniform
+}
+
+// T2m: lower median (rank (n-1)/2 of the ascending values) of the window x4[0 .. n/4), by the whole team; every
+// lane of a team with `need` returns it (teams without `need` just keep the warp together).  mu / sigma (floats)
+// only guide the first pivots.  The values are only read.
+template <int G>
+__device__ float f32f_median(const float4* x4, int n, const F32Quads& Q, float muf, float sigf, bool need,
+                             F32FastCtx<G>& c) {
+  constexpr uint32_t CAP = (uint32_t)f32f_cap<G>();
   const float* x = reinterpret_cast<const float*>(x4);
-  const uint32_t rho = (uint32_t)(n - 1) >> 1;
+  const uint32_t rho = need ? (uint32_t)(n - 1) >> 1 : 0u;
   const float inf = __int_as_float(0x7f800000);
   // invariant: #{v <= a} = ca <= rho < cb = #{v <= b}; the answer is the (rho - ca)-th smallest value in (a, b]
   float a = -inf, b = inf;
-  uint32_t ca = 0, cb = (uint32_t)n;
+  uint32_t ca = 0, cb = need ? (uint32_t)n : 0u;
   // first pivots: the median of n Gaussian draws is within 1.25 sigma / sqrt(n) (one standard deviation) of mu
-  float R = 3.2f * sigf * rsqrtf((float)n);
+  float R = 3.2f * sigf * rsqrtf((float)max(n, 1));
   float p1 = muf - R, p2 = muf + R;
-  for (int pass = 0; pass < 64 && cb - ca > (uint32_t)f32f_cap<G>(); ++pass) {
+  bool done = !need;                                     // result known without gathering
+  float result = 0.0f;
+  bool searching = need && cb - ca > CAP;
+  for (int pass = 0; pass < 64 && f32f_any<G>(searching); ++pass) {
     if (!(p1 > a)) p1 = a;                               // keep the pivots inside the bracket (also rejects NaN)
     if (!(p2 < b)) p2 = b;
     if (!(p1 <= p2)) p1 = p2;
-    uint32_t c1 = 0, c12 = 0;                            // #{v <= p1}, #{v <= p1} + #{v <= p2}
-    f32f_each_quad<G>(Q, c.j, [&](int qi, int) {
+    uint32_t c1 = 0, c2 = 0;                             // #{v <= p1}, #{v <= p2}
+    uint32_t c1a = 0, c1b = 0, c2a = 0, c2b = 0;
+    F32Quads Qs = Q;
+    if (!searching) { Qs.T = 0; Qs.t0 = 0; }
+    f32f_each_quad<G>(Qs, c.j, [&](int qi, int) {
       const float4 v = x4[qi];
-      const uint32_t a0 = v.x <= p1, a1 = v.y <= p1, a2 = v.z <= p1, a3 = v.w <= p1;
-      const uint32_t b0 = v.x <= p2, b1 = v.y <= p2, b2 = v.z <= p2, b3 = v.w <= p2;
-      c1 += a0 + a1; c1 += a2 + a3;
-      c12 += b0 + b1; c12 += b2 + b3;
+      c1a -= f32f_le_mask(v.x, p1) + f32f_le_mask(v.y, p1);
+      c1b -= f32f_le_mask(v.z, p1) + f32f_le_mask(v.w, p1);
+      c2a -= f32f_le_mask(v.x, p2) + f32f_le_mask(v.y, p2);
+      c2b -= f32f_le_mask(v.z, p2) + f32f_le_mask(v.w, p2);
     });
+    c1 = c1a + c1b; c2 = c2a + c2b;
     // one reduction for both counts: n <= 2^15 in this kernel (the host checks), so each fits 16 bits
-    const uint32_t packed = f32f_sum_u32<G>(c1 | (c12 << 16), c);
-    c1 = packed & 0xffffu;
-    const uint32_t c2 = packed >> 16;
-    if (rho < c1) { b = p1; cb = c1; }
-    else if (rho < c2) { a = p1; ca = c1; b = p2; cb = c2; }
-    else { a = p2; ca = c2; }
-    const uint32_t m = cb - ca;
-    if (m <= (uint32_t)f32f_cap<G>()) break;
-    // next pivots
-    if (a > -inf && b < inf && b > a) {
-      // interpolate the rank inside (a, b] and step aside by a margin of a few binomial standard deviations
-      const float w = b - a;
-      if (!(w <= 3.0e38f)) break;                        // (unreachable for |x| < 1e18: key bisection below)
-      const float f = ((float)(rho - ca) + 0.5f) / (float)m;
-      const float dev = (2.0f * sqrtf(f * (1.0f - f) * (float)m) + 1.0f) / (float)m;
-      p1 = a + w * fmaxf(f - dev, 0.0f);
-      p2 = a + w * fminf(f + dev, 1.0f);
-      if (!(p1 > a)) p1 = f32_next_up(a);                // the float grid is exhausted towards a
-      if (!(p1 < b)) return b;                           // a and b are neighbouring floats: every value in (a, b] is b
-      if (!(p2 < b)) p2 = f32_next_down(b);
-      if (!(p2 >= p1)) p2 = p1;
-    } else if (b == inf && a == -inf) {                  // (both pivots collapsed: cannot happen, but stay finite)
-      p1 = muf - 2.0f * R; p2 = muf + 2.0f * R; R *= 2.0f;
-    } else if (b == inf) {                               // everything seen so far lies below the rank: go up
-      R *= 4.0f;
-      p1 = a + R; p2 = a + 4.0f * R;
-      if (!(p1 > a)) { p1 = 3.402823466e38f; p2 = 3.402823466e38f; }
-      if (!(p2 < inf)) p2 = 3.402823466e38f;
-    } else {                                             // a == -inf: go down
-      R *= 4.0f;
-      p2 = b - R; p1 = b - 4.0f * R;
-      if (!(p2 < b)) { p1 = -3.402823466e38f; p2 = -3.402823466e38f; }
-      if (!(p1 > -inf)) p1 = -3.402823466e38f;
+    const uint32_t packed = f32f_sum_u32<G>(c1 | (c2 << 16), c);
+    if (searching) {
+      c1 = packed & 0xffffu;
+      c2 = packed >> 16;
+      if (rho < c1) { b = p1; cb = c1; }
+      else if (rho < c2) { a = p1; ca = c1; b = p2; cb = c2; }
+      else { a = p2; ca = c2; }
+      const uint32_t m = cb - ca;
+      if (m <= CAP) {
+        searching = false;
+      } else if (a > -inf && b < inf) {
+        // interpolate the rank inside (a, b] and step aside by a margin of a few binomial standard deviations
+        const float w = b - a;
+        const float f = ((float)(rho - ca) + 0.5f) / (float)m;
+        const float dev = (2.0f * sqrtf(f * (1.0f - f) * (float)m) + 1.0f) / (float)m;
+        p1 = a + w * fmaxf(f - dev, 0.0f);
+        p2 = a + w * fminf(f + dev, 1.0f);
+        if (!(p1 > a)) p1 = f32_next_up(a);              // the float grid is exhausted towards a
+        if (!(p2 < b)) p2 = f32_next_down(b);
+        if (!(p2 >= p1)) p2 = p1;
+        if (!(w <= 3.0e38f)) {                           // (unreachable for |x| < 1e18) -> key bisection below
+          searching = false;
+        } else if (!(p1 < b)) {                          // a and b are neighbouring floats: every value in (a, b] is b
+          searching = false; done = true; result = b;
+        }
+      } else if (b == inf && a == -inf) {                // (both pivots collapsed: cannot happen, but stay finite)
+        R *= 2.0f;
+        p1 = muf - R; p2 = muf + R;
+      } else if (b == inf) {                             // everything seen so far lies below the rank: go up
+        R *= 4.0f;
+        p1 = a + R; p2 = a + 4.0f * R;
+        if (!(p1 > a)) { p1 = 3.402823466e38f; p2 = 3.402823466e38f; }
+        if (!(p2 < inf)) p2 = 3.402823466e38f;
+      } else {                                           // a == -inf: go down
+        R *= 4.0f;
+        p2 = b - R; p1 = b - 4.0f * R;
+        if (!(p2 < b)) { p1 = -3.402823466e38f; p2 = -3.402823466e38f; }
+        if (!(p1 > -inf)) p1 = -3.402823466e38f;
+      }
     }
   }
-  const uint32_t m = cb - ca;
-  if (m > (uint32_t)f32f_cap<G>()) {
-    // last resort (64 passes did not shrink the bracket: a pathological value distribution): bisection on the
-    // order-preserving integer keys, 32 counting passes, always terminates
+  // last resort (the bracket did not shrink in 64 passes: a pathological value distribution): bisection on the
+  // order-preserving integer keys, 32 counting passes, always terminates
+  bool bisect = need && !done && cb - ca > CAP;
+  if (f32f_any<G>(bisect)) {
     uint32_t klo = 0u, khi = 0xffffffffu;
-    while (klo < khi) {
+    for (int step = 0; step < 32; ++step) {              // 32 halvings of a 2^32 range
       const uint32_t mid = klo + ((khi - klo) >> 1);
       uint32_t cnt = 0;
-      f32f_each_quad<G>(Q, c.j, [&](int qi, int) {
+      F32Quads Qs = Q;
+      if (!bisect) { Qs.T = 0; Qs.t0 = 0; }
+      f32f_each_quad<G>(Qs, c.j, [&](int qi, int) {
         const float4 v = x4[qi];
         cnt += (f32_key(v.x) <= mid) + (f32_key(v.y) <= mid) + (f32_key(v.z) <= mid) + (f32_key(v.w) <= mid);
       });
       cnt = f32f_sum_u32<G>(cnt, c);
       if (cnt > rho) khi = mid; else klo = mid + 1;
     }
-    const uint32_t bits = (klo & 0x80000000u) ? (klo & 0x7fffffffu) : ~klo;
-    return __int_as_float((int)bits);
+    if (bisect) {
+      const uint32_t bits = (klo & 0x80000000u) ? (klo & 0x7fffffffu) : ~klo;
+      result = __int_as_float((int)bits);
+      done = true;
+    }
   }
-  // gather the (at most 32) elements of (a, b] as indices, then rank them: the one with rank rho - ca is the median
+  // gather the (at most CAP) elements of (a, b] as indices, then rank them: the one with rank rho - ca is the median
+  const bool gather = need && !done;
+  const uint32_t m = gather ? cb - ca : 0u;
   if (c.j == 0) c.T->ln = 0;
   f32f_sync<G>(c);
-  f32f_each_quad<G>(Q, c.j, [&](int qi, int) {
-    const float4 v = x4[qi];
-    // a quad holds a value of (a, b] only if ... cheap necessary test first: most quads hold none
-    const bool in0 = v.x > a && v.x <= b, in1 = v.y > a && v.y <= b, in2 = v.z > a && v.z <= b, in3 = v.w > a && v.w <= b;
-    if (in0 | in1 | in2 | in3) {
-      if (in0) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi);
-      if (in1) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 1);
-      if (in2) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 2);
-      if (in3) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 3);
-    }
-  });
+  {
+    F32Quads Qs = Q;
+    if (!gather) { Qs.T = 0; Qs.t0 = 0; }
+    f32f_each_quad<G>(Qs, c.j, [&](int qi, int) {
+      const float4 v = x4[qi];
+      const bool in0 = v.x > a && v.x <= b, in1 = v.y > a && v.y <= b, in2 = v.z > a && v.z <= b, in3 = v.w > a && v.w <= b;
+      if (in0 | in1 | in2 | in3) {
+        if (in0) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi);
+        if (in1) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 1);
+        if (in2) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 2);
+        if (in3) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 3);
+      }
+    });
+  }
   f32f_sync<G>(c);
   const uint32_t want = rho - ca;
   for (uint32_t i = (uint32_t)c.j; i < m; i += G) {
@@ -232,28 +274,31 @@ __device__ float f32f_median(const float4* x4, int n, const F32Quads& Q, float m
     if (rank == want) c.T->result = e;
   }
   f32f_sync<G>(c);
-  const float r = c.T->result;
+  if (gather) result = c.T->result;
   f32f_sync<G>(c);                                       // nobody reads the scratch after this point
-  return r;
+  return result;
 }
 
-// One window, all thresholds, by one team.  x4 points at the window in shared memory, n is a multiple of 4.
+// One window, all thresholds, by one team.  x4 points at the window in shared memory, n is a multiple of 4; a team
+// without a window (valid = false: more teams than windows in this round) only keeps its warp together.
 template <int G>
-__device__ __forceinline__ void f32f_window(float4* x4, int n, const TdF32Params& P, uint8_t* flags, int team_in_warp,
-                                            F32FastCtx<G>& c) {
-  const int nq = n >> 2;
+__device__ __forceinline__ void f32f_window(float4* x4, int n, bool valid, const TdF32Params& P, uint8_t* flags,
+                                            int team_in_warp, F32FastCtx<G>& c) {
+  const int nq = valid ? n >> 2 : 0;
   F32Quads Q;
   Q.T = nq > c.j ? (nq - c.j + G - 1) / G : 0;
   Q.t0 = 0;
   if (G < 8 && Q.T > 0) Q.t0 = (team_in_warp & (8 / G - 1)) % Q.T;
   const float* xs = reinterpret_cast<const float*>(x4);
   // ---------------------------------------------------------------- T2: statistics around the pivot
-  double piv = (double)xs[0];
+  double piv = valid ? (double)xs[0] : 0.0;
   double A = 0.0, B = 0.0;
-  const double rn = 1.0 / (double)n;
-  auto sums = [&]() {
+  const double rn = 1.0 / (double)(valid ? n : 1);
+  auto sums = [&](bool mine) {
     double A0 = 0.0, B0 = 0.0, A1 = 0.0, B1 = 0.0;
-    f32f_each_quad<G>(Q, c.j, [&](int qi, int) {
+    F32Quads Qs = Q;
+    if (!mine) { Qs.T = 0; Qs.t0 = 0; }
+    f32f_each_quad<G>(Qs, c.j, [&](int qi, int) {
       const float4 v = x4[qi];
       const double d0 = (double)v.x - piv, d1 = (double)v.y - piv, d2 = (double)v.z - piv, d3 = (double)v.w - piv;
       A0 += d0; B0 = fma(d0, d0, B0);
@@ -261,15 +306,22 @@ __device__ __forceinline__ void f32f_window(float4* x4, int n, const TdF32Params
       A0 += d2; B0 = fma(d2, d2, B0);
       A1 += d3; B1 = fma(d3, d3, B1);
     });
-    A = A0 + A1; B = B0 + B1;
-    f32f_sum2<G>(A, B, c);
+    double a2 = A0 + A1, b2 = B0 + B1;
+    f32f_sum2<G>(a2, b2, c);
+    if (mine) { A = a2; B = b2; }
   };
   auto cancels = [&]() {                                 // team-uniform
     const double am = A * rn, m2 = B * rn;
     return m2 - am * am < 1e-6 * m2;
   };
-  sums();
-  if (cancels()) { piv += A * rn; sums(); }
+  sums(true);
+  {
+    const bool again = valid && cancels();
+    if (f32f_any<G>(again)) {
+      if (again) piv += A * rn;
+      sums(again);
+    }
+  }
 
   bool have_median = false;
   float median = 0.0f;
@@ -291,7 +343,7 @@ __device__ __forceinline__ void f32f_window(float4* x4, int n, const TdF32Params
       if (hi > t_hi || lo < t_lo) fm |= 1u << t;
     });
     uint32_t cnt = 0;
-    if (fm) {
+    {
       uint32_t f2 = fm;
       while (f2) {
         const int t = __ffs(f2) - 1;
@@ -302,18 +354,14 @@ __device__ __forceinline__ void f32f_window(float4* x4, int n, const TdF32Params
       }
     }
     cnt = f32f_sum_u32<G>(cnt, c);
-    if (cnt == 0) continue;                              // team-uniform
+    const bool flagged = cnt != 0;                       // team-uniform
     // ---------------------------------------------------------------- T2m / replacement value
-    float r;
-    if (P.policy == 0) {
-      r = (float)mu;
-    } else {
-      if (!have_median) {
-        median = f32f_median<G>(x4, n, Q, (float)mu, (float)sigma, c);
-        have_median = true;
-      }
-      r = median;
+    const bool need_med = flagged && P.policy != 0 && !have_median;
+    if (f32f_any<G>(need_med)) {
+      const float med = f32f_median<G>(x4, n, Q, (float)mu, (float)sigma, need_med, c);
+      if (need_med) { median = med; have_median = true; }
     }
+    const float r = P.policy == 0 ? (float)mu : median;
     // ---------------------------------------------------------------- T4: replace, T5: deltas
     double dA = 0.0, dB = 0.0;
     const double dr = (double)r - piv;
@@ -335,19 +383,20 @@ __device__ __forceinline__ void f32f_window(float4* x4, int n, const TdF32Params
       }
       x4[qi] = v;
     }
-    if (it + 1 < P.n_thr) {
-      f32f_sum2<G>(dA, dB, c);                           // (for G <= 32 the shuffles also order the team's writes)
+    if (it + 1 < P.n_thr && f32f_any<G>(flagged)) {
+      f32f_sum2<G>(dA, dB, c);
       const double B_before = B;
       A += dA; B += dB;
       // sum again around the current mean when the update cannot be trusted: the mean has left the pivot behind, or
       // the replaced samples carried nearly all of B (a 1e8 sigma spike: B was 1e16 + the rest, in 53 bits)
-      if (cancels() || B < 1e-6 * B_before) {
-        f32f_sync<G>(c);
-        piv += A * rn;
-        sums();
+      const bool again = flagged && (cancels() || B < 1e-6 * B_before);
+      if (f32f_any<G>(again)) {
+        f32f_sync<G>(c);                                 // the team's replacements are visible
+        if (again) piv += A * rn;
+        sums(again);
       }
     }
-    if (c.j == 0 && P.counts) atomicAdd(&P.counts[it], (unsigned long long)cnt);
+    if (flagged && c.j == 0 && P.counts) atomicAdd(&P.counts[it], (unsigned long long)cnt);
   }
 }
 
@@ -397,10 +446,13 @@ __global__ void __launch_bounds__(kF32FastThreads, 4) td_f32_fast_kernel(const T
     phase ^= 1;
     // ---------------------------------------------------------------- T2..T5: windows of the row
     uint8_t* fl = P.flags ? P.flags + row * P.S : nullptr;
-    for (int w = c.team; w < nwin; w += NT) {
-      const int w0 = w * P.window;
-      f32f_window<G>(reinterpret_cast<float4*>(slot + w0), min(P.window, P.S - w0), P, fl ? fl + w0 : nullptr,
-                     team_in_warp, c);
+    for (int wb = 0; wb < nwin; wb += NT) {             // a round of NT windows: warp-uniform trip count
+      const int w = wb + c.team;
+      const bool valid = w < nwin;
+      if (G >= 32 && !valid) continue;                   // (a team of whole warps may simply skip)
+      const int w0 = valid ? w * P.window : 0;
+      f32f_window<G>(reinterpret_cast<float4*>(slot + w0), valid ? min(P.window, P.S - w0) : 0, valid, P,
+                     fl ? fl + w0 : nullptr, team_in_warp, c);
     }
     // ---------------------------------------------------------------- T6: store
     fence_proxy_async_smem();
