@@ -405,12 +405,22 @@ TABLE_CASES = [
     ("cfg3 FDSC u8 {4,3} in place", 3, "freq", {}, True),
     ("cfg3 FDSC u8 bins of 32, {2.75,2.75} out of place", 3, "freq", {"bin_size": 32, "ks": [2.75, 2.75]}, False),
     ("cfg3 FDSC u8 bins of 32, {2.75,2.75} in place", 3, "freq", {"bin_size": 32, "ks": [2.75, 2.75]}, True),
+    ("cfg3 FDSC u8 {4,3} median, in place", 3, "freq", {"policy": "median"}, True),
+    ("cfg4 x 96 beams FDSC u8 {4,3} in place", 4, "freq", {"beams": 96, "ks": [4.0, 3.0]}, True),
+    ("cfg4 x 96 beams FDSC u8 {4,3} out of place", 4, "freq", {"beams": 96, "ks": [4.0, 3.0]}, False),
+    ("cfg4 x 96 beams FDSC u8 bins of 32, {2.75,2.75} in place", 4, "freq",
+     {"beams": 96, "bin_size": 32, "ks": [2.75, 2.75]}, True),
+    ("cfg4 x 96 beams TDSC u8 {5,4,3} median", 4, "time", {"beams": 96, "policy": "median"}, False),
     ("cfg5 TDSC f32 W=256 median", 5, "time", {"window": 256}, False),
     ("cfg5 TDSC f32 W=1024 median", 5, "time", {"window": 1024}, False),
     ("cfg5 TDSC f32 W=12500 median", 5, "time", {"window": 12500}, False),
     ("cfg5 TDSC f32 W=256 mean", 5, "time", {"window": 256, "policy": "mean"}, False),
     ("cfg5 TDSC f32 W=1024 mean", 5, "time", {"window": 1024, "policy": "mean"}, False),
     ("cfg5 TDSC f32 W=12500 mean", 5, "time", {"window": 12500, "policy": "mean"}, False),
+    ("cfg5-shaped FDSC f32 {4,3} mean", 5, "freq", {"policy": "mean"}, False),
+    ("cfg5-shaped FDSC f32 {4,3} median", 5, "freq", {"policy": "median"}, False),
+    ("cfg5-shaped FDSC f32 bins of 32, {2.75,2.75} mean", 5, "freq", {"policy": "mean", "bin_size": 32, "ks": [2.75, 2.75]},
+     False),
 ]
 
 
@@ -432,7 +442,7 @@ def run_table(quiet: bool = False, only: str = ""):
     for (label, n, op, kw, inplace) in TABLE_CASES:
         if only and only not in label:
             continue
-        cfg = synth.config(n)
+        cfg = synth.config(n, **({"beams": kw["beams"]} if "beams" in kw else {}))
         if n not in inputs:
             inputs.clear()
             torch.cuda.empty_cache()

@@ -29,30 +29,31 @@ namespace rfim {
 
 constexpr int kFqWarps = 4;
 constexpr int kFqThreads = 32 * kFqWarps;
-constexpr int kFqSlots = 4;                          // boxes per warp ring (the statistics loop is unrolled by it)
+constexpr int kFqMaxRing = 4;                        // boxes per warp ring (3 and 5 measured slower)
 constexpr int kFqListCap = 256;                      // candidate blocks per warp and repair chunk
 
 struct __align__(16) FqCtrl {
   uint32_t acc[2][2 * kFsCols];                      // [buffer][S of 128 columns | Q of 128 columns]
   uint8_t lo[kFsCols], hi[kFsCols], rr[kFsCols];
-  uint64_t full[kFqWarps][kFqSlots];                 // ring mbarriers
+  uint64_t full[kFqWarps][kFqMaxRing];               // ring mbarriers
   int tk[3][4];                                      // tile tickets handed to this CTA: {tile, beam, tile in beam}
   uint16_t list[kFqWarps][kFqListCap];               // candidate blocks of a warp: block << 5 | lane
 };
-// shared memory of one CTA: [rings: 4 warps x 4 boxes][summaries: 4 warps x NBQ x 32 lanes x 16 bytes][FqCtrl]
-__host__ __device__ inline size_t fd_quad_smem_bytes(int nbq) {
-  return (size_t)kFqWarps * kFqSlots * kFsBoxWords * 4 + (size_t)kFqWarps * nbq * 32 * 16 + sizeof(FqCtrl);
+// shared memory of one CTA: [rings: 4 warps x `ring` boxes][summaries: 4 warps x NBQ x 32 lanes x 16 bytes][FqCtrl]
+__host__ __device__ inline size_t fd_quad_smem_bytes(int nbq, int ring) {
+  return (size_t)kFqWarps * ring * kFsBoxWords * 4 + (size_t)kFqWarps * nbq * 32 * 16 + sizeof(FqCtrl);
 }
 
-// NBQ = boxes per warp and tile / 4 (C = 128 NBQ channels); kCopy: out of place
-template <int NBQ, bool kCopy>
-__global__ void __launch_bounds__(kFqThreads, 4) fd_u8_quad_kernel(const __grid_constant__ FdStreamMaps maps,
+// NBQ = boxes per warp and tile / 4 (C = 128 NBQ channels); kCopy: out of place; kRing: boxes per warp ring
+template <int NBQ, bool kCopy, int kRing>
+__global__ void __launch_bounds__(kFqThreads, kRing == 3 ? 5 : 4) fd_u8_quad_kernel(const __grid_constant__ FdStreamMaps maps,
                                                                    const FdStreamParams P) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr int NB = 4 * NBQ;                        // boxes of 8 class rows per warp and tile
   constexpr int NW = (NBQ + 3) / 4;                  // 32-bit words of candidate bits per lane (8 bits per 4 boxes)
   const int tid = threadIdx.x, lane = tid & 31, cls = tid >> 5;
   const int C = P.C;
+  constexpr int kFqSlots = kRing;
   uint32_t* const ring = reinterpret_cast<uint32_t*>(smem) + (size_t)cls * kFqSlots * kFsBoxWords;
   uint4* const sum4 = reinterpret_cast<uint4*>(smem + (size_t)kFqWarps * kFqSlots * kFsBoxWords * 4) + (size_t)cls * NBQ * 32;
   FqCtrl* const K = reinterpret_cast<FqCtrl*>(smem + (size_t)kFqWarps * kFqSlots * kFsBoxWords * 4 +
@@ -97,6 +98,7 @@ __global__ void __launch_bounds__(kFqThreads, 4) fd_u8_quad_kernel(const __grid_
   }
 
   uint32_t phases = 0;                                // one parity bit per ring slot
+  int slot = 0;                                       // ring slot of the next box (boxes follow one another across tiles)
   int buf = 0;                                        // accumulator buffer of the next exchange
   uint32_t colS = 0, colQ = 0;                        // thread = column: exact totals, kept across iterations
   const int offw = P.off[cls] >> 2;                   // word offset of column s0 inside a box row
@@ -121,10 +123,11 @@ __global__ void __launch_bounds__(kFqThreads, 4) fd_u8_quad_kernel(const __grid_
     for (int q = 0; q < NBQ; ++q) {
       uint32_t mx0 = 0, mx1 = 0, mn0 = 0, mn1 = 0;    // summaries of the 8 blocks of these 4 boxes
 #pragma unroll
-      for (int u = 0; u < kFqSlots; ++u) {            // box c = 4 q + u lives in ring slot u
+      for (int u = 0; u < 4; ++u) {                   // box c = 4 q + u lives in ring slot `slot`
         const int c = 4 * q + u;
-        mbar_wait(&full[u], (phases >> u) & 1u);
-        const uint32_t* rowp = ring + u * kFsBoxWords + offw + lane;
+        mbar_wait(&full[slot], (phases >> slot) & 1u);
+        phases ^= 1u << slot;
+        const uint32_t* rowp = ring + slot * kFsBoxWords + offw + lane;
         uint32_t w[kFsBoxRows];
 #pragma unroll
         for (int j = 0; j < kFsBoxRows; ++j) w[j] = rowp[j * kFsPitchW];
@@ -160,11 +163,11 @@ __global__ void __launch_bounds__(kFqThreads, 4) fd_u8_quad_kernel(const __grid_
         // loads have completed (re-arming earlier lets the asynchronous copy overtake them).
         __syncwarp();
         if (lane == 0) {
-          if (c + kFqSlots < NB) issue(s0, cur_y0, c + kFqSlots, u);
-          else if (have_next) issue(nxt_s0, nxt_y0, c + kFqSlots - NB, u);
+          if (c + kFqSlots < NB) issue(s0, cur_y0, c + kFqSlots, slot);
+          else if (have_next) issue(nxt_s0, nxt_y0, c + kFqSlots - NB, slot);
         }
+        slot = (slot + 1 == kFqSlots) ? 0 : slot + 1;
       }
-      phases ^= (1u << kFqSlots) - 1u;
       sum4[q * 32 + lane] = make_uint4(mx0, mx1, mn0, mn1);
     }
 #pragma unroll

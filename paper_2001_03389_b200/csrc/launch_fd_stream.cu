@@ -117,10 +117,13 @@ int launch_fd_stream(const Call& c, const StreamPlan& pl, int sms) {
 // ---- one warp per alignment class (fd_u8_quad.cuh): one bin, channel counts of 128 * {4, 8, 12, 16}
 template <int NBQ>
 int launch_fd_quad_n(const Call& c, bool copy, const rfim::FdStreamMaps& maps, const rfim::FdStreamParams& P, int sms) {
+  // a ring of 4 boxes per warp and four CTAs per SM (measured on config 4: 3.63 ms; a ring of 3 with five CTAs per
+  // SM 3.76 ms, a ring of 5 3.79 ms)
+  constexpr int ring = 4;
   void (*kernel)(const rfim::FdStreamMaps, const rfim::FdStreamParams) =
-      copy ? rfim::fd_u8_quad_kernel<NBQ, true> : rfim::fd_u8_quad_kernel<NBQ, false>;
+      copy ? rfim::fd_u8_quad_kernel<NBQ, true, ring> : rfim::fd_u8_quad_kernel<NBQ, false, ring>;
   const char* name = copy ? "fd_u8_quad_copy" : "fd_u8_quad";
-  const size_t smem = rfim::fd_quad_smem_bytes(NBQ);
+  const size_t smem = rfim::fd_quad_smem_bytes(NBQ, ring);
   int st = ensure_smem(kernel, smem);
   if (st != RFIM_OK) return st;
   int occ = 0;

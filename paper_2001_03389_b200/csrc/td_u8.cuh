@@ -13,10 +13,10 @@
 //       the groups it found by itself (exact per-byte masks, replace, S and Q deltas, summary
 //       refresh), so there is no queue, atomic or barrier.  T5: next threshold, on chip, from the
 //       updated S, Q and summaries.  T6: one TMA bulk store.  HBM sees one read and one write per
-//       sample.  Median replacement (kMedian): the replacement value of an iteration is the lower
-//       median of the snapshot, found -- only in rows where the iteration cuts something, at the first hit and
-//       therefore before any replacement -- by counting passes over the staged row (bytes <= v, packed compares
-//       + IDP.4A) that start at the rounded mean and bracket, then bisect, the rank.
+//       sample.  Median replacement (kMedian): the replacement value is the lower median of the
+//       snapshot, found -- only in rows where an iteration cuts something, at the first hit and therefore before
+//       any replacement -- by counting passes over the staged row (bytes <= v, packed compares + IDP.4A) that start
+//       at the rounded mean and bracket, then bisect, the rank; it is the same for every later iteration.
 //   td_u8_generic_kernel  any alignment / stride / row length / window, mean or median: one CTA per
 //       row, byte loads, iterations through global memory (L1/L2).  Correctness path, not tuned.
 #pragma once
@@ -266,6 +266,8 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
 
     // ---------------------------------------------------------------- T3..T5: thresholds, on chip
     uint4* s4w = reinterpret_cast<uint4*>(slot);
+    bool have_med = false;                                         // kMedian: the row's lower median, once known
+    uint32_t med = 0;
     for (int it = 0; it < P.n_thr; ++it) {
       // T3: exact kept interval [lo, hi] for this snapshot (every warp of the team computes the same
       // scalars: cheaper than another barrier)
@@ -316,7 +318,13 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
         if (!have_r) {
           // first hit of this iteration: nothing has been replaced yet, the slot still holds the snapshot
           r = rounded_mean_u8((uint32_t)S, Ssum);
-          if (kMedian) r = warp_lower_median_u8(s4, J, S, h, geo.pe, xf, xl, r, lane);
+          if (kMedian) {
+            // The lower median is taken ONCE per row: replacing samples by the lower median m never changes it (with
+            // L samples < m and E samples = m, L <= rank < L + E; moving l samples from below and u from above onto
+            // m leaves L - l <= rank < L + E + u), so every later iteration's snapshot median is the same m.
+            if (!have_med) { med = warp_lower_median_u8(s4, J, S, h, geo.pe, xf, xl, r, lane); have_med = true; }
+            r = med;
+          }
           r4 = r * 0x01010101u;
           have_r = true;
         }
