@@ -91,6 +91,11 @@ bool tensor_maps_available();
 bool encode_class_maps(const uint8_t* base, int64_t stride, int samples, int64_t rows, int box_w, int box_rows,
                        CUtensorMapL2promotion promo, ClassMaps& out);
 
+// a plain 2-D tensor map over [rows][cols] float32 with row pitch `pitch_bytes` (a multiple of 16, base 16-byte
+// aligned), box = box_cols x box_rows elements
+bool encode_f32_map(const float* base, int64_t pitch_bytes, int cols, int64_t rows, int box_cols, int box_rows,
+                    CUtensorMap& out);
+
 // the launch units (each returns an rfim_status; RFIM_ERR_UNSUPPORTED = no kernel of that family takes the call)
 int launch_td_u8(const Call& c);
 int launch_td_f32(const Call& c);

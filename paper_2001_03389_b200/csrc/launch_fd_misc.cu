@@ -3,6 +3,7 @@
 #include "host.h"
 #include "fd_u8.cuh"
 #include "fd_f32.cuh"
+#include "fd_f32_tile.cuh"
 #include "fd_u8_binned.cuh"
 
 namespace rfim_host {
@@ -75,7 +76,62 @@ int launch_fd_u8(const Call& c) {
 }
 
 // ------------------------------------------------------------------------------------------ FD f32
+// the resident-tile kernel (fd_f32_tile.cuh): one bin, all channels x 32 samples per tile in shared memory
+int try_fd_f32_tile(const Call& c, int sms) {
+  if (c.bin_size != c.channels) return RFIM_ERR_UNSUPPORTED;
+  const uintptr_t a = reinterpret_cast<uintptr_t>(c.data) | reinterpret_cast<uintptr_t>(c.out);
+  if ((a & 15) != 0 || c.stride % 4 != 0) return RFIM_ERR_UNSUPPORTED;          // tensor maps: 16-byte pitch and base
+  if (c.channels < 2 || c.channels > 32768) return RFIM_ERR_UNSUPPORTED;
+  const size_t smem = rfim::fd_f32_tile_smem_bytes(c.channels);
+  if (smem > (size_t)kMaxSmem) return RFIM_ERR_UNSUPPORTED;
+  if (!tensor_maps_available()) return RFIM_ERR_UNSUPPORTED;
+  int box_rows = 0;                                                            // largest divisor of C up to 256
+  for (int d = 256; d >= 1; --d)
+    if (c.channels % d == 0) { box_rows = d; break; }
+  const int nboxes = c.channels / box_rows;
+  if (nboxes > rfim::kFtMaxBoxes) return RFIM_ERR_UNSUPPORTED;
+  if ((int64_t)c.beams * c.channels > 0x7fffffff) return RFIM_ERR_UNSUPPORTED;  // tensor coordinates
+  rfim::FdF32TileParams P;
+  memset(&P, 0, sizeof(P));
+  P.src = static_cast<const float*>(c.data);
+  P.dst = static_cast<float*>(c.out);
+  P.stride = c.stride;
+  P.beams = c.beams; P.C = c.channels; P.S = c.samples;
+  P.n_thr = c.n_thr;
+  P.policy = (int)c.policy;
+  for (int i = 0; i < c.n_thr; ++i) P.k[i] = c.thr[i];
+  P.flags = c.flags;
+  P.counts = c.counts;
+  P.box_rows = box_rows; P.nboxes = nboxes;
+  P.tiles_per_beam = (c.samples + rfim::kFtCols - 1) / rfim::kFtCols;
+  P.total_tiles = (int64_t)P.tiles_per_beam * c.beams;
+  P.copy = c.out != c.data ? 1 : 0;
+  rfim::FdF32TileMaps maps;
+  memset(&maps, 0, sizeof(maps));
+  const int64_t rows = (int64_t)c.beams * c.channels;
+  if (!encode_f32_map(P.src, c.stride * 4, c.samples, rows, rfim::kFtCols, box_rows, maps.src)) return RFIM_ERR_UNSUPPORTED;
+  if (!encode_f32_map(P.dst, c.stride * 4, c.samples, rows, rfim::kFtCols, box_rows, maps.dst)) return RFIM_ERR_UNSUPPORTED;
+  auto kernel = rfim::fd_f32_tile_kernel;
+  int st = ensure_smem(kernel, smem);
+  if (st != RFIM_OK) return st;
+  int occ = 0;
+  if ((st = blocks_per_sm(kernel, rfim::kFtThreads, smem, occ)) != RFIM_OK) return st;
+  if (occ < 1) return RFIM_ERR_UNSUPPORTED;
+  int64_t grid = P.total_tiles;
+  if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
+  if ((st = clear_outputs(c)) != RFIM_OK) return st;
+  return launch(P.policy ? "fd_f32_tile_median" : "fd_f32_tile", kernel, dim3((unsigned)grid), dim3(rfim::kFtThreads),
+                smem, c.stream, 0, maps, P);
+}
+
 int launch_fd_f32(const Call& c) {
+  if (c.variant == 0 || c.variant == 2) {
+    int sms0 = 0;
+    int st0 = sm_count(sms0);
+    if (st0 != RFIM_OK) return st0;
+    st0 = try_fd_f32_tile(c, sms0);
+    if (st0 != RFIM_ERR_UNSUPPORTED) return st0;
+  }
   rfim::FdF32Params P;
   memset(&P, 0, sizeof(P));
   P.src = static_cast<const float*>(c.data);

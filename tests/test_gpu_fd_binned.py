@@ -78,7 +78,10 @@ def check_policy(x_np, ks, bin_size, policy):
     flags = torch.zeros(x_np.shape, dtype=torch.uint8, device=DEV)
     counts = torch.zeros(len(ks), dtype=torch.int64, device=DEV)
     out = torch.empty_like(x)
-    rfim.rfim_freq_sigma_cut(x, ks, policy, out=out, bin_size=bin_size, flags=flags, counts=counts)
+    # float32: the definition kernel (variant 1), whose fp64 operations follow the oracle's order exactly; the tuned
+    # float32 kernel has its own test module (test_gpu_fd_f32_tile.py)
+    rfim.rfim_freq_sigma_cut(x, ks, policy, out=out, bin_size=bin_size, flags=flags, counts=counts,
+                             variant=rfim.VARIANT_GENERIC if x_np.dtype == np.float32 else rfim.VARIANT_AUTO)
     torch.cuda.synchronize()
     got = out.cpu().numpy()
     if x_np.dtype == np.uint8:

@@ -22,9 +22,7 @@ def fast_name(C, S, inplace=False):
     """The tuned kernel auto mode picks for a dense [.][C][S] uint8 request with mean replacement and one bin."""
     if S % 4 != 0:
         return "fd_u8_generic"
-    if C in (512, 1024, 1536, 2048):
-        return "fd_u8_stream" if inplace else "fd_u8_stream_copy"
-    return "fd_u8_strip"
+    return "fd_u8_strip"          # short batches: the resident-tile kernel (large ones in place: fd_u8_quad)
 
 
 def run_gpu(x_np, ks, variant=rfim.VARIANT_AUTO, inplace=False, pitch=None, want_flags=True):
@@ -274,10 +272,10 @@ def test_strip_cluster_sizes(C, name):
     x[0, ::97, :] = 250
     x[1, C // 2:C // 2 + 40, 17:60] = 0
     x[1, :, 299] = 7
-    got, _ = check(x, [4.0, 3.0], variant=STRIP)       # (auto prefers the streaming kernel for 1024 / 1536 channels)
+    got, _ = check(x, [4.0, 3.0], variant=STRIP)
     assert got == name
-    got, _ = check(x, [4.0, 3.0])
-    assert got == ("fd_u8_stream_copy" if C in (1024, 1536) else name)
+    got, _ = check(x, [4.0, 3.0])                      # auto: short batches go to the strip kernel too
+    assert got == name
     check(x, [0.5, 3.0, 3.0], inplace=True, variant=STRIP)
     got, _ = check(x, [4.0, 3.0], variant=STRIP_BULK)  # the same kernel with per-row bulk copies
     assert got == name.replace("_bulk", "") + "_bulk"
