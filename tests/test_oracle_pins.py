@@ -631,3 +631,35 @@ def test_out_of_place_stride_and_errors():
     # zero thresholds: a valid no-op
     y, f, c = oracle.time_sigma_cut(x, [])
     assert np.array_equal(y, x) and f.sum() == 0
+
+
+# ----------------------------------------------------------------------------------------------------------------
+# R22: with median replacement the snapshot median never changes from one iteration to the next --
+# with L samples < m and E samples = m (L <= rank < L + E), replacing l samples from below and u from above by m
+# leaves L - l <= rank < L + E + u.  The kernels take the median once per row / window / column on the strength of
+# this; here the recomputing oracle is checked against the property (it is a theorem about the definition, so a
+# failure would mean a wrong median or replacement step in the oracle).
+@pytest.mark.parametrize("dtype", ["u8", "f32"])
+def test_r22_median_is_invariant_under_median_replacement(dtype):
+    rng = np.random.default_rng(22)
+    for trial in range(40):
+        n = int(rng.integers(5, 400))
+        if dtype == "u8":
+            row = np.clip(np.rint(rng.normal(100, 12, n)), 0, 255)
+            row[rng.random(n) < 0.08] = rng.integers(0, 256)
+            x = row.astype(np.uint8).reshape(1, 1, n)
+        else:
+            row = rng.normal(0, 1, n)
+            row[rng.random(n) < 0.08] *= 30.0
+            x = row.astype(np.float32).reshape(1, 1, n)
+        ks = [float(k) for k in rng.choice([1.0, 1.5, 2.0, 3.0], size=4)]
+        med = np.sort(x[0, 0])[(n - 1) // 2]
+        out, flags, counts = oracle.time_sigma_cut(x, ks, policy=oracle.MEDIAN)
+        assert np.all(out[0, 0][flags[0, 0] != 0] == med), (trial, ks)
+        # the same along the channel axis, per bin
+        nb = int(rng.choice([0, 1]))
+        xc = np.ascontiguousarray(x.reshape(1, n, 1))
+        outc, flagsc, _ = oracle.freq_sigma_cut(xc, ks, policy=oracle.MEDIAN)
+        assert np.all(outc[0, :, 0][flagsc[0, :, 0] != 0] == med)
+        if sum(int(c) for c in counts) > 0:
+            assert np.sort(out[0, 0])[(n - 1) // 2] == med          # and the cleaned row still has that median
