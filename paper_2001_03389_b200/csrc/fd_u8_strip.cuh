@@ -88,6 +88,8 @@ struct __align__(16) FdStripCtrl {
   uint4 chk[kStripWords];                        // per word column {negE, negO, thrE, thrO}
   uint8_t lo[kStripCols], hi[kStripCols], rr[kStripCols];
   uint64_t bar[32];                              // tensor path: one per alignment class, or one per warp (kWarpBox); bulk path: bar[0]
+  uint32_t cnt[kStripCols];                      // kMedian: samples above the probe value, per column
+  uint8_t mid[kStripCols];                       // kMedian: probe value of the bisection, per column
 };
 __host__ __device__ inline size_t fd_strip_smem_bytes(int Rq) {
   return (size_t)Rq * kStripPitchW * 4 + sizeof(FdStripCtrl);
@@ -107,7 +109,9 @@ __device__ __forceinline__ void smem_red_add(uint32_t* p, uint32_t v) {
 // kWarpBox (tensor path, Rq a multiple of 8 NW): a warp owns Rq / NW CONSECUTIVE rows of its alignment class, one
 // tensor box with its own mbarrier, so every warp runs its own copy-in / store / next-copy-in pipeline and no warp
 // waits for the slowest warp of its class before the next tile's rows are requested.
-template <bool kTensor, int NW, bool kWarpBox>
+// kMedian (single CTA per tile only): the replacement value is the column's lower median, found once
+// per column on the resident tile by bisection over the byte values with packed counting passes.
+template <bool kTensor, int NW, bool kWarpBox, bool kMedian = false>
 __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(const __grid_constant__ FdStripMaps maps,
                                                                                 const FdStripParams P) {
   constexpr int kStripThreads = 32 * NW, kStripWarps = NW;
@@ -180,6 +184,7 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
   uint32_t phase = 0;
   int buf = 0;                                        // accumulator buffer of the next exchange
   uint32_t colS = 0, colQ = 0;                        // owner: exact column totals, kept across iterations
+  uint32_t med_col = 0;                               // owner, kMedian: the column's lower median
   for (int64_t t = cluster_id_x(); t < P.total_tiles; t += nclusters) {
     const int b = (int)(t / P.tiles_per_beam);
     const int s0 = (int)(t % P.tiles_per_beam) * kStripCols;
@@ -258,6 +263,7 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
             thread_bounds_u8_sqrt(cut, lo, hi);
             r = rounded_mean_u8((uint32_t)C, colS);
           }
+          if (kMedian && !first) r = med_col;                         // (first: the search below fills it in)
         }
         const int u = ocol & 3, slot = (u & 1) * 2 + (u >> 1);       // E.lo, O.lo, E.hi, O.hi
         const uint32_t neg = (0x10000u - ((uint32_t)lo << 8)) & 0xffffu;
@@ -319,6 +325,45 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
       }
     }
     if (P.n_thr > 0) exchange(true, 0);
+    if (kMedian && P.n_thr > 0) {
+      // T2m on the resident tile, once per column (the lower median does not change when samples are replaced by
+      // it: DESIGN.md R22).  |median - mean| <= sigma always, so the search starts from [mean - sigma - 1, mean +
+      // sigma + 1]; a step counts, per column, the samples above the probe value (packed compare, one byte counter
+      // per column and thread) and halves the interval: the smallest v with #{x <= v} > rank is the lower median.
+      const uint32_t rank_m = (uint32_t)(C - 1) >> 1;
+      int vlo = 0, vhi = 0;
+      if (owner && ocol < tw) {
+        const uint64_t V = (uint64_t)C * colQ - (uint64_t)colS * colS;
+        const float rc = 1.0f / (float)C;
+        const float mu = (float)colS * rc, sg = sqrtf((float)V) * rc;
+        vlo = max(0, (int)floorf(mu - sg) - 1);
+        vhi = min(255, (int)ceilf(mu + sg) + 1);
+      }
+      while (true) {
+        const bool active = owner && vlo < vhi;
+        if (owner) { K->mid[ocol] = (uint8_t)((vlo + vhi) >> 1); K->cnt[ocol] = 0; }
+        if (!__syncthreads_or(active)) break;                        // (also publishes the probes)
+        if (ni > 0) {
+          const uint32_t mid4 = reinterpret_cast<const uint32_t*>(K->mid)[lane];
+          const uint32_t chiE = 0x7fff7fffu - prmt_b32(mid4, 0u, 0x4240u), chiO = 0x7fff7fffu - prmt_b32(mid4, 0u, 0x4341u);
+          uint32_t above4 = 0;                                        // per column: samples > probe (ni <= 255)
+          const uint32_t* col = col0;
+#pragma unroll 4
+          for (int i = 0; i < ni; ++i, col += RS)
+            above4 += bytes_outside_cols(col[0], chiE, 0x80008000u, chiO, 0x80008000u) & 0x01010101u;
+#pragma unroll
+          for (int u = 0; u < 4; ++u) smem_red_add(&K->cnt[4 * lane + u], (above4 >> (8 * u)) & 0xffu);
+        }
+        __syncthreads();
+        if (active) {
+          const uint32_t le = (uint32_t)C - K->cnt[ocol];
+          const int mid = (vlo + vhi) >> 1;
+          if (le > rank_m) vhi = mid; else vlo = mid + 1;
+        }
+      }
+      if (owner) { med_col = (uint32_t)vlo; K->rr[ocol] = (uint8_t)vlo; }
+      __syncthreads();
+    }
 
     // Tensor path, full-width tile: the LAST sweep writes the rows it finds clean straight from its registers
     // (F6 fused into F4: no second pass over shared memory for them); repaired rows are written by the repair.

@@ -15,7 +15,8 @@ int strip_box_rows(int rq) {
   return 0;
 }
 bool plan_fd_u8_strip(const Call& c, bool want_tensor, int force_cl, StripPlan& pl) {
-  if (c.policy != RFIM_REPLACE_MEAN || c.bin_size != c.channels) return false;
+  if (c.bin_size != c.channels) return false;
+  const bool median = c.policy == RFIM_REPLACE_MEDIAN;           // the median search runs inside ONE CTA per tile
   const uintptr_t src = reinterpret_cast<uintptr_t>(c.data), dst = reinterpret_cast<uintptr_t>(c.out);
   if ((src & 3) != 0 || (c.stride & 3) != 0) return false;       // 32-bit word columns
   if (((src ^ dst) & 15) != 0) return false;                     // aligned interiors of src and dst rows coincide
@@ -28,6 +29,7 @@ bool plan_fd_u8_strip(const Call& c, bool want_tensor, int force_cl, StripPlan& 
     for (int cl = 1; cl <= 8; cl *= 2) {
       if (pass == 0 && (cl != 1 || force_cl < 0)) continue;
       if (force_cl > 0 && cl != force_cl) continue;
+      if (median && cl != 1) continue;
       const int rq = (c.channels + cl - 1) / cl;
       if (rq > 255 * 16) continue;                               // packed per-thread delta counters (255 rows/thread)
       // tensor copies: every CTA holds whole alignment classes, the rows of a CTA start at a multiple of 4 in the
@@ -74,9 +76,14 @@ int launch_fd_strip(const Call& c, const StripPlan& pl, int sms) {
     for (int k = 0; k < 4; ++k) { maps.src[k] = cm.m[k]; P.off[k] = cm.off[k]; }
     P.box_rows = pl.box_rows;
   }
+  const bool median = c.policy == RFIM_REPLACE_MEDIAN;
   auto kernel = pl.nw == 16 ? (pl.tensor ? rfim::fd_u8_strip_kernel<true, 16, false> : rfim::fd_u8_strip_kernel<false, 16, false>)
                 : pl.warp_box ? rfim::fd_u8_strip_kernel<true, 32, true>
                               : (pl.tensor ? rfim::fd_u8_strip_kernel<true, 32, false> : rfim::fd_u8_strip_kernel<false, 32, false>);
+  if (median)
+    kernel = pl.nw == 16 ? (pl.tensor ? rfim::fd_u8_strip_kernel<true, 16, false, true> : rfim::fd_u8_strip_kernel<false, 16, false, true>)
+             : pl.warp_box ? rfim::fd_u8_strip_kernel<true, 32, true, true>
+                           : (pl.tensor ? rfim::fd_u8_strip_kernel<true, 32, false, true> : rfim::fd_u8_strip_kernel<false, 32, false, true>);
   int st = ensure_smem(kernel, (size_t)pl.smem);
   if (st != RFIM_OK) return st;
   int nclusters = 0;
@@ -89,7 +96,8 @@ int launch_fd_strip(const Call& c, const StripPlan& pl, int sms) {
   if ((st = clear_outputs(c)) != RFIM_OK) return st;
   static const char* names[2][4] = {{"fd_u8_strip1_bulk", "fd_u8_strip2_bulk", "fd_u8_strip4_bulk", "fd_u8_strip8_bulk"},
                                     {"fd_u8_strip1", "fd_u8_strip2", "fd_u8_strip4", "fd_u8_strip8"}};
-  return launch(names[pl.tensor][pl.cl == 1 ? 0 : pl.cl == 2 ? 1 : pl.cl == 4 ? 2 : 3], kernel,
+  static const char* mnames[2] = {"fd_u8_strip1_bulk_median", "fd_u8_strip1_median"};
+  return launch(median ? mnames[pl.tensor] : names[pl.tensor][pl.cl == 1 ? 0 : pl.cl == 2 ? 1 : pl.cl == 4 ? 2 : 3], kernel,
                 dim3((unsigned)(want * pl.cl)), dim3((unsigned)(32 * pl.nw)), (size_t)pl.smem, c.stream, pl.cl, maps, P);
 }
 

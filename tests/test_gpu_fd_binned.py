@@ -100,7 +100,9 @@ def test_median_replacement_u8(C, S, nb):
     replacement is the lower median of the bin."""
     x = banded((2, C, S), seed=C + S + nb)
     name, counts = check_policy(x, [3.0, 3.0], nb, "median")
-    assert name == "fd_u8_binned_generic"
+    # one bin on 4-byte aligned rows: the strip kernel finds the median on its resident tile; bins: the definition
+    assert name == ("fd_u8_strip1_bulk_median" if nb == 0 and S % 4 == 0 and C % 4 != 0 else
+                    "fd_u8_strip1_median" if nb == 0 and S % 4 == 0 else "fd_u8_binned_generic"), name
     check_policy(x, [1.0], nb, "median")
 
 

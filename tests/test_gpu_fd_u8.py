@@ -256,7 +256,7 @@ def test_zero_thresholds_is_copy():
 def test_unsupported_requests_fail_loudly():
     x = torch.zeros((1, 64, 128), dtype=torch.uint8, device=DEV)
     with pytest.raises(rfim.RfimError) as e:
-        rfim.rfim_freq_sigma_cut(x, [3.0], policy="median", variant=TILE)   # no fast kernel for the median policy
+        rfim.rfim_freq_sigma_cut(x, [3.0], policy="median", bin_size=16, variant=TILE)   # no tuned kernel for median with bins
     assert e.value.status == -2
 
 
@@ -281,3 +281,50 @@ def test_strip_cluster_sizes(C, name):
     assert got == name.replace("_bulk", "") + "_bulk"
     got, _ = check(x, [4.0, 3.0], variant=STRIP_CLUSTER)   # never the whole tile in one CTA: clusters, two CTAs per SM
     assert got.startswith("fd_u8_strip2" if C in (1536, 1537, 1028, 1024, 1280, 1152) else name.replace("_bulk", ""))
+
+
+# ----------------------------------------------------------------------------------- median replacement (NEXT-3)
+def check_median(x_np, ks, inplace=False, variant=rfim.VARIANT_AUTO, want=None):
+    ref, rflags, rcounts = oracle.freq_sigma_cut(x_np, ks, policy=oracle.MEDIAN)
+    x = torch.from_numpy(x_np).to(DEV)
+    out = None if inplace else torch.full_like(x, 0xAB)
+    flags = torch.full(x_np.shape, 7, dtype=torch.uint8, device=DEV)
+    counts = torch.full((len(ks),), -1, dtype=torch.int64, device=DEV)
+    res = rfim.rfim_freq_sigma_cut(x, ks, "median", out=out, flags=flags, counts=counts, variant=variant)
+    torch.cuda.synchronize()
+    name = rfim.rfim_last_variant()
+    got = res.cpu().numpy()
+    assert np.array_equal(got, ref), f"{name}: cleaned array differs at {np.argwhere(got != ref)[:5]}"
+    assert np.array_equal(flags.cpu().numpy(), rflags), f"{name}: flags differ"
+    assert counts.cpu().tolist() == [int(c) for c in rcounts], f"{name}: counts"
+    if want:
+        assert name == want, name
+    return name
+
+
+@pytest.mark.parametrize("C,S,want", [(1536, 300, "fd_u8_strip1_median"), (1536, 128, "fd_u8_strip1_median"),
+                                      (512, 212, "fd_u8_strip1_median"), (64, 100, "fd_u8_strip1_median"),
+                                      (30, 44, "fd_u8_strip1_bulk_median"), (2, 64, "fd_u8_strip1_bulk_median"),
+                                      (4096, 140, "fd_u8_binned_generic")])
+def test_median_replacement_in_the_strip_kernel(C, S, want):
+    """FDSC with the median strategy on the resident tile: the lower median of every column by
+    bisection over the byte values, once per column; the oracle recomputes it in every iteration.  4096 channels
+    do not fit one CTA: the definition kernel."""
+    x = noisy((2, C, S), seed=C + S)
+    if C >= 8:
+        x[0, C // 2, :] = np.minimum(x[0, C // 2, :].astype(int) + 90, 255).astype(np.uint8)   # narrow-band RFI
+        x[1, ::3, S // 2] = 255                       # a third of a column saturated: median far from the noise
+        x[1, C - 1, S - 1] = 0
+        x[0, :, 0] = 77                               # constant column
+        x[0, : C // 2, 1] = 10                        # two-level column with an even split (lower median = 10)
+        x[0, C // 2:, 1] = 200
+    check_median(x, [4.0, 3.0], want=want)
+    check_median(x, [3.25, 3.25, 3.25], inplace=True, want=want)
+    check_median(x, [0.5, 1.0, 2.0, 3.0], inplace=True, want=want)     # k < 1: the kept interval may miss the median
+
+
+def test_median_config3_slice():
+    cfg = synth.config(3, beams=2)
+    x = synth.fill_host(cfg, beam0=3, beams=2)
+    check_median(x, cfg["thresholds"], inplace=True, want="fd_u8_strip1_median")
+    check_median(x[:1], [2.75, 2.75], want="fd_u8_strip1_median")
