@@ -48,16 +48,15 @@
  *
  * Performance notes (DESIGN.md section 6 and BASELINE.md section 4 have the numbers).  Tuned kernels exist for:
  *   uint8 TDSC on whole rows of <= 65000 samples, mean or median;
- *   uint8 FDSC, one bin, mean (any channel count that is a multiple of 4) or median (tiles that fit one CTA:
- *     up to about 1570 channels); mean only: 512 / 1024 / 1536 / 2048
- *     channels take the streaming kernel on large in-place batches) or bins whose size is a multiple of 16 and
- *     divides channels / 4 (for 512 / 1024 / 1536 / 2048 channels);
+ *   uint8 FDSC, one bin, mean (any channel count that is a multiple of 4) or median (tiles that fit one CTA: up
+ *     to about 1570 channels); 512 / 1024 / 1536 / 2048 channels with mean replacement take a streaming kernel on
+ *     large in-place batches, and also accept bins whose size is a multiple of 16 and divides channels / 4;
  *   float32 TDSC on rows that fit shared memory (<= about 56000 samples) with windows that are multiples of 4
  *     samples (or the whole row), 16-byte aligned rows, mean or median;
  *   float32 FDSC, one bin, mean or median, 16-byte aligned rows, channels x 128 bytes <= about 220 KB.
  * Everything else the ABI accepts (uint8 TDSC with windows or rows longer than 65000 samples, uint8 FDSC with median
- * replacement and bins, or odd bin sizes, float32 FDSC with bins, unaligned float32 rows) runs in definition kernels (one
- * thread per column / one CTA per row) that go through L2 several times: 10 to 50 times slower.
+ * replacement and bins, or odd bin sizes, float32 FDSC with bins, unaligned float32 rows) runs in definition
+ * kernels (one thread per column / one CTA per row) that go through L2 several times: 10 to 50 times slower.
  */
 #ifndef RFIM_H
 #define RFIM_H
