@@ -38,7 +38,11 @@ struct __align__(8) F32FastTeam {
   uint16_t list[kF32FastListCap];   // gathered candidates: element indices inside the window
   int ln;                           // gather cursor
   float result;
+  int rec;                          // CTA-wide median search: this team's entry in the request list
+  int pad;
 };
+// CTA-wide median search (one window per team and row): a request per window that needs its median
+struct __align__(8) F32FastSel { int w0, n; float mu, sig, result; int pad; };
 // exchange area of the teams that span several warps (G >= 64): at most 4 teams x 8 warps
 struct __align__(16) F32FastXchg {
   double red[2][8][2];
@@ -49,6 +53,7 @@ __host__ __device__ inline size_t f32_fast_smem_bytes(int S, int G) {
   size_t b = ((size_t)S * 4 + 15) & ~(size_t)15;
   b += (size_t)f32_fast_teams(G) * sizeof(F32FastTeam);
   if (G > 32) b = ((b + 15) & ~(size_t)15) + (size_t)f32_fast_teams(G) * sizeof(F32FastXchg);
+  b = ((b + 15) & ~(size_t)15) + (size_t)f32_fast_teams(G) * sizeof(F32FastSel) + 16;   // requests + two counters
   return b + 16;
 }
 
@@ -61,6 +66,12 @@ struct F32FastCtx {
   int team;           // team index inside the CTA
   int lane, wt;       // lane inside the warp, warp inside the team
   int sel;            // exchange buffer
+  // CTA-wide median search
+  F32FastTeam* teams; // scratch of team 0
+  F32FastSel* req;    // request list
+  int* nreq;          // two counters, used alternately
+  const float* slot;  // the staged row
+  int ncall;          // calls so far (CTA-uniform)
 };
 
 template <int G>
@@ -279,9 +290,169 @@ __device__ float f32f_median(const float4* x4, int n, const F32Quads& Q, float m
   return result;
 }
 
+// The same search by a team of Gv lanes chosen at run time (4 <= Gv <= 32, lanes vmask of one warp); every warp of
+// the CTA calls it together, teams without a window (act = false) only keep their warp converged.
+__device__ inline float f32f_median_rt(const float4* x4, int n, int jv, int Gv, uint32_t vmask, F32FastTeam* T, float muf,
+                                float sigf, bool act) {
+  const float* x = reinterpret_cast<const float*>(x4);
+  const uint32_t CAP = Gv <= 4 ? 12u : (Gv <= 16 ? 16u : 32u);
+  const int nq = act ? n >> 2 : 0;
+  const uint32_t rho = act ? (uint32_t)(n - 1) >> 1 : 0u;
+  const float inf = __int_as_float(0x7f800000);
+  auto sum_u32 = [&](uint32_t v) {
+    for (int o = Gv >> 1; o > 0; o >>= 1) v += __shfl_xor_sync(vmask, v, o);
+    return v;
+  };
+  float a = -inf, b = inf;
+  uint32_t ca = 0, cb = act ? (uint32_t)n : 0u;
+  float R = 3.2f * sigf * rsqrtf((float)max(n, 1));
+  float p1 = muf - R, p2 = muf + R;
+  bool done = !act;
+  float result = 0.0f;
+  bool searching = act && cb - ca > CAP;
+  for (int pass = 0; pass < 64 && __any_sync(FULL, searching); ++pass) {
+    if (!(p1 > a)) p1 = a;
+    if (!(p2 < b)) p2 = b;
+    if (!(p1 <= p2)) p1 = p2;
+    uint32_t c1a = 0, c1b = 0, c2a = 0, c2b = 0;
+    const int nqs = searching ? nq : 0;
+#pragma unroll 2
+    for (int qi = jv; qi < nqs; qi += Gv) {
+      const float4 v = x4[qi];
+      c1a -= f32f_le_mask(v.x, p1) + f32f_le_mask(v.y, p1);
+      c1b -= f32f_le_mask(v.z, p1) + f32f_le_mask(v.w, p1);
+      c2a -= f32f_le_mask(v.x, p2) + f32f_le_mask(v.y, p2);
+      c2b -= f32f_le_mask(v.z, p2) + f32f_le_mask(v.w, p2);
+    }
+    const uint32_t packed = sum_u32((c1a + c1b) | ((c2a + c2b) << 16));
+    if (searching) {
+      const uint32_t c1 = packed & 0xffffu, c2 = packed >> 16;
+      if (rho < c1) { b = p1; cb = c1; }
+      else if (rho < c2) { a = p1; ca = c1; b = p2; cb = c2; }
+      else { a = p2; ca = c2; }
+      const uint32_t m = cb - ca;
+      if (m <= CAP) {
+        searching = false;
+      } else if (a > -inf && b < inf) {
+        const float w = b - a;
+        const float f = ((float)(rho - ca) + 0.5f) / (float)m;
+        const float dev = (2.0f * sqrtf(f * (1.0f - f) * (float)m) + 1.0f) / (float)m;
+        p1 = a + w * fmaxf(f - dev, 0.0f);
+        p2 = a + w * fminf(f + dev, 1.0f);
+        if (!(p1 > a)) p1 = f32_next_up(a);
+        if (!(p2 < b)) p2 = f32_next_down(b);
+        if (!(p2 >= p1)) p2 = p1;
+        if (!(w <= 3.0e38f)) searching = false;
+        else if (!(p1 < b)) { searching = false; done = true; result = b; }
+      } else if (b == inf && a == -inf) {
+        R *= 2.0f;
+        p1 = muf - R; p2 = muf + R;
+      } else if (b == inf) {
+        R *= 4.0f;
+        p1 = a + R; p2 = a + 4.0f * R;
+        if (!(p1 > a)) { p1 = 3.402823466e38f; p2 = 3.402823466e38f; }
+        if (!(p2 < inf)) p2 = 3.402823466e38f;
+      } else {
+        R *= 4.0f;
+        p2 = b - R; p1 = b - 4.0f * R;
+        if (!(p2 < b)) { p1 = -3.402823466e38f; p2 = -3.402823466e38f; }
+        if (!(p1 > -inf)) p1 = -3.402823466e38f;
+      }
+    }
+  }
+  const bool bisect = act && !done && cb - ca > CAP;
+  if (__any_sync(FULL, bisect)) {
+    uint32_t klo = 0u, khi = 0xffffffffu;
+    for (int step = 0; step < 32; ++step) {
+      const uint32_t mid = klo + ((khi - klo) >> 1);
+      uint32_t cnt = 0;
+      const int nqs = bisect ? nq : 0;
+      for (int qi = jv; qi < nqs; qi += Gv) {
+        const float4 v = x4[qi];
+        cnt += (f32_key(v.x) <= mid) + (f32_key(v.y) <= mid) + (f32_key(v.z) <= mid) + (f32_key(v.w) <= mid);
+      }
+      cnt = sum_u32(cnt);
+      if (cnt > rho) khi = mid; else klo = mid + 1;
+    }
+    if (bisect) {
+      const uint32_t bits = (klo & 0x80000000u) ? (klo & 0x7fffffffu) : ~klo;
+      result = __int_as_float((int)bits);
+      done = true;
+    }
+  }
+  const bool gather = act && !done;
+  const uint32_t m = gather ? cb - ca : 0u;
+  if (act && jv == 0) T->ln = 0;
+  __syncwarp(vmask);
+  {
+    const int nqs = gather ? nq : 0;
+    for (int qi = jv; qi < nqs; qi += Gv) {
+      const float4 v = x4[qi];
+      const bool in0 = v.x > a && v.x <= b, in1 = v.y > a && v.y <= b, in2 = v.z > a && v.z <= b, in3 = v.w > a && v.w <= b;
+      if (in0 | in1 | in2 | in3) {
+        if (in0) T->list[atomicAdd(&T->ln, 1)] = (uint16_t)(4 * qi);
+        if (in1) T->list[atomicAdd(&T->ln, 1)] = (uint16_t)(4 * qi + 1);
+        if (in2) T->list[atomicAdd(&T->ln, 1)] = (uint16_t)(4 * qi + 2);
+        if (in3) T->list[atomicAdd(&T->ln, 1)] = (uint16_t)(4 * qi + 3);
+      }
+    }
+  }
+  __syncwarp(vmask);
+  const uint32_t want = rho - ca;
+  for (uint32_t i = (uint32_t)jv; i < m; i += (uint32_t)Gv) {
+    const uint32_t ii = T->list[i];
+    const float e = x[ii];
+    uint32_t rank = 0;
+    for (uint32_t k = 0; k < m; ++k) {
+      const uint32_t kk = T->list[k];
+      const float o = x[kk];
+      rank += (o < e) || (o == e && kk < ii);
+    }
+    if (rank == want) T->result = e;
+  }
+  __syncwarp(vmask);
+  if (gather) result = T->result;
+  __syncwarp(vmask);
+  return result;
+}
+
+// CTA-wide median search (every thread of the CTA calls it): the windows that need their median are listed, the
+// 256 lanes are re-divided evenly among them (32, 16, 8 or 4 lanes per window), each such team runs the search on
+// its window, and the owners pick their result up.  Half the windows of a row need no median at k = 3: this keeps
+// every lane busy during the search instead of every second team.
+template <int G>
+__device__ float f32f_cta_median(int w0, int n, float muf, float sigf, bool need, F32FastCtx<G>& c) {
+  const int tid = threadIdx.x;
+  int* const cnt = &c.nreq[c.ncall & 1];
+  if (need && c.j == 0) {
+    const int my = atomicAdd(cnt, 1);
+    F32FastSel r;
+    r.w0 = w0; r.n = n; r.mu = muf; r.sig = sigf; r.result = 0.0f; r.pad = 0;
+    c.req[my] = r;
+    c.T->rec = my;
+  }
+  __syncthreads();
+  if (tid == 0) c.nreq[(c.ncall + 1) & 1] = 0;         // the counter of the previous call: everybody is past it
+  ++c.ncall;
+  const int K = *cnt;
+  int Gv = 32;
+  while (Gv * K > kF32FastThreads) Gv >>= 1;           // K <= 256 / G <= 64, so Gv >= 4
+  const int v = tid / Gv, jv = tid % Gv;
+  const bool act = v < K;
+  const F32FastSel r = c.req[act ? v : 0];
+  const uint32_t vmask = Gv == 32 ? FULL : (((1u << Gv) - 1u) << (c.lane & ~(Gv - 1)));
+  const float med = f32f_median_rt(reinterpret_cast<const float4*>(c.slot + r.w0), r.n, jv, Gv, vmask,
+                                   c.teams + (act ? v : 0), r.mu, r.sig, act);
+  if (act && jv == 0) c.req[v].result = med;
+  __syncthreads();
+  return need ? c.req[c.T->rec].result : 0.0f;
+}
+
 // One window, all thresholds, by one team.  x4 points at the window in shared memory, n is a multiple of 4; a team
 // without a window (valid = false: more teams than windows in this round) only keeps its warp together.
-template <int G>
+// kCta: every team of the CTA is inside this function at the same time (one window per team and row), so the median
+// search may be CTA-wide.
+template <int G, bool kCta>
 __device__ __forceinline__ void f32f_window(float4* x4, int n, bool valid, const TdF32Params& P, uint8_t* flags,
                                             int team_in_warp, F32FastCtx<G>& c) {
   const int nq = valid ? n >> 2 : 0;
@@ -357,7 +528,13 @@ __device__ __forceinline__ void f32f_window(float4* x4, int n, bool valid, const
     const bool flagged = cnt != 0;                       // team-uniform
     // ---------------------------------------------------------------- T2m / replacement value
     const bool need_med = flagged && P.policy != 0 && !have_median;
-    if (f32f_any<G>(need_med)) {
+    if (kCta) {
+      if (__syncthreads_or(need_med)) {
+        const int w0 = (int)(reinterpret_cast<const float*>(x4) - c.slot);
+        const float med = f32f_cta_median<G>(w0, n, (float)mu, (float)sigma, need_med, c);
+        if (need_med) { median = med; have_median = true; }
+      }
+    } else if (f32f_any<G>(need_med)) {
       const float med = f32f_median<G>(x4, n, Q, (float)mu, (float)sigma, need_med, c);
       if (need_med) { median = med; have_median = true; }
     }
@@ -415,6 +592,11 @@ __global__ void __launch_bounds__(kF32FastThreads, 4) td_f32_fast_kernel(const T
     xchg = reinterpret_cast<F32FastXchg*>(smem + off);
     off += (size_t)NT * sizeof(F32FastXchg);
   }
+  off = (off + 15) & ~(size_t)15;
+  F32FastSel* req = reinterpret_cast<F32FastSel*>(smem + off);
+  off += (size_t)NT * sizeof(F32FastSel);
+  int* nreq = reinterpret_cast<int*>(smem + off);
+  off += 16;
   uint64_t* bar = reinterpret_cast<uint64_t*>(smem + ((off + 7) & ~(size_t)7));
   const int tid = threadIdx.x, lane = tid & 31;
   F32FastCtx<G> c;
@@ -426,6 +608,8 @@ __global__ void __launch_bounds__(kF32FastThreads, 4) td_f32_fast_kernel(const T
   c.T = teams + c.team;
   c.X = G > 32 ? xchg + c.team : nullptr;
   c.tmask = G >= 32 ? FULL : (((1u << (G & 31)) - 1u) << (lane & ~(G - 1)));
+  c.teams = teams; c.req = req; c.nreq = nreq; c.slot = slot; c.ncall = 0;
+  if (tid < 2) nreq[tid] = 0;
   const int team_in_warp = G >= 32 ? 0 : (lane / G);
   if (tid == 0) {
     mbar_init(bar, 1);
@@ -446,13 +630,22 @@ __global__ void __launch_bounds__(kF32FastThreads, 4) td_f32_fast_kernel(const T
     phase ^= 1;
     // ---------------------------------------------------------------- T2..T5: windows of the row
     uint8_t* fl = P.flags ? P.flags + row * P.S : nullptr;
-    for (int wb = 0; wb < nwin; wb += NT) {             // a round of NT windows: warp-uniform trip count
-      const int w = wb + c.team;
+    if (G < kF32FastThreads && nwin <= NT && P.policy != 0) {
+      // one window per team: all teams work side by side, the median search is CTA-wide
+      const int w = c.team;
       const bool valid = w < nwin;
-      if (G >= 32 && !valid) continue;                   // (a team of whole warps may simply skip)
       const int w0 = valid ? w * P.window : 0;
-      f32f_window<G>(reinterpret_cast<float4*>(slot + w0), valid ? min(P.window, P.S - w0) : 0, valid, P,
-                     fl ? fl + w0 : nullptr, team_in_warp, c);
+      f32f_window<G, true>(reinterpret_cast<float4*>(slot + w0), valid ? min(P.window, P.S - w0) : 0, valid, P,
+                           fl ? fl + w0 : nullptr, team_in_warp, c);
+    } else {
+      for (int wb = 0; wb < nwin; wb += NT) {           // a round of NT windows: warp-uniform trip count
+        const int w = wb + c.team;
+        const bool valid = w < nwin;
+        if (G >= 32 && !valid) continue;                 // (a team of whole warps may simply skip)
+        const int w0 = valid ? w * P.window : 0;
+        f32f_window<G, false>(reinterpret_cast<float4*>(slot + w0), valid ? min(P.window, P.S - w0) : 0, valid, P,
+                              fl ? fl + w0 : nullptr, team_in_warp, c);
+      }
     }
     // ---------------------------------------------------------------- T6: store
     fence_proxy_async_smem();
