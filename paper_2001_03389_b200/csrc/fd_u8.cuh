@@ -3,7 +3,7 @@
 // distributed-shared-memory wrappers used by the strip kernel) and
 //   fd_u8_generic_kernel  any pitch / alignment / channel count: one thread per (beam, sample) column,
 //       iterations through global memory (L2).  Correctness path for the shapes the fast kernels
-//       (fd_u8_stream.cuh, fd_u8_strip.cuh) do not take; not tuned.
+//       (fd_u8_quad.cuh, fd_u8_stream.cuh, fd_u8_strip.cuh) do not take; not tuned.
 #pragma once
 
 #include "common.cuh"

@@ -2,7 +2,9 @@
 // one bin of all channels: the strip kernel.
 //
 // The general fast kernel: any channel count that is a multiple of 4 (up to ~12 K channels through clusters of
-// CTAs).  The streaming kernel of fd_u8_stream.cuh is preferred for the channel counts it takes.
+// CTAs), mean replacement, or -- for tiles that fit one CTA -- the median (kMedian).  Auto mode takes it for short
+// batches and out of place; large in-place batches go to the streaming kernel of fd_u8_quad.cuh, bins to
+// fd_u8_stream.cuh (launch_fd_misc.cu has the order and the measurements behind it).
 //
 // A tile is ALL channels x 128 consecutive samples of one beam (a strip), resident in shared memory as rows of
 // 144 bytes.  Whenever it fits (<= 1576 channels) ONE CTA of 32 warps holds the whole tile (216 KB, one CTA per
