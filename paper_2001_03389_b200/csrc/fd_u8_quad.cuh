@@ -266,11 +266,9 @@ __global__ void __launch_bounds__(kFqThreads, kRing == 3 ? 5 : 4) fd_u8_quad_ker
         }
         __syncwarp();
         const int n = min(total, kFqListCap);
-        // one entry = one block: 4 class rows x the 4 bytes of word column L.  The words of the NEXT round are
+        // one entry = one block: 4 class rows x the 4 bytes of word column L.  The words of the next TWO rounds are
         // requested before this round's are examined, so a round costs its instructions, not an L2 round trip.
-        uint32_t w4[4] = {0, 0, 0, 0};
-        uint32_t ent = 0;
-        auto fetch = [&](int e) {
+        auto fetch = [&](int e, uint32_t& ent, uint32_t (&w4)[4]) {
           if (e < n) {
             ent = list[e];
             const int nvL = tw - 4 * (int)(ent & 31u);
@@ -287,12 +285,17 @@ __global__ void __launch_bounds__(kFqThreads, kRing == 3 ? 5 : 4) fd_u8_quad_ker
             }
           }
         };
-        fetch(lane);
+        uint32_t entA = 0, entB = 0, wA[4] = {0, 0, 0, 0}, wB[4] = {0, 0, 0, 0};
+        fetch(lane, entA, wA);
+        fetch(32 + lane, entB, wB);
         for (int e0 = 0; e0 < n; e0 += 32) {
           const bool have = e0 + lane < n;
-          const uint32_t cent = ent;
-          const uint32_t c0 = w4[0], c1 = w4[1], c2 = w4[2], c3 = w4[3];
-          fetch(e0 + 32 + lane);
+          const uint32_t cent = entA;
+          const uint32_t c0 = wA[0], c1 = wA[1], c2 = wA[2], c3 = wA[3];
+          entA = entB;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) wA[i] = wB[i];
+          fetch(e0 + 64 + lane, entB, wB);
           if (have) {
             const int L = (int)(cent & 31u), blk = (int)(cent >> 5);
             const int nv = tw - 4 * L;                                // valid bytes of that word column
