@@ -31,6 +31,7 @@ constexpr int kFqWarps = 4;
 constexpr int kFqThreads = 32 * kFqWarps;
 constexpr int kFqMaxRing = 4;                        // boxes per warp ring (3 and 5 measured slower)
 constexpr int kFqAhead = 0;                          // L2 prefetch distance in boxes; 0 = off (12 measured: 4.23 vs 3.63 ms)
+constexpr int kFqDepth = 3;                          // repair rounds whose loads are in flight
 constexpr int kFqListCap = 256;                      // candidate blocks per warp and repair chunk
 
 struct __align__(16) FqCtrl {
@@ -266,7 +267,7 @@ __global__ void __launch_bounds__(kFqThreads, kRing == 3 ? 5 : 4) fd_u8_quad_ker
         }
         __syncwarp();
         const int n = min(total, kFqListCap);
-        // one entry = one block: 4 class rows x the 4 bytes of word column L.  The words of the next TWO rounds are
+        // one entry = one block: 4 class rows x the 4 bytes of word column L.  The words of the next kFqDepth rounds are
         // requested before this round's are examined, so a round costs its instructions, not an L2 round trip.
         auto fetch = [&](int e, uint32_t& ent, uint32_t (&w4)[4]) {
           if (e < n) {
@@ -285,17 +286,25 @@ __global__ void __launch_bounds__(kFqThreads, kRing == 3 ? 5 : 4) fd_u8_quad_ker
             }
           }
         };
-        uint32_t entA = 0, entB = 0, wA[4] = {0, 0, 0, 0}, wB[4] = {0, 0, 0, 0};
-        fetch(lane, entA, wA);
-        fetch(32 + lane, entB, wB);
+        uint32_t ents[kFqDepth], ws[kFqDepth][4];
+#pragma unroll
+        for (int d = 0; d < kFqDepth; ++d) {
+          ents[d] = 0;
+#pragma unroll
+          for (int i = 0; i < 4; ++i) ws[d][i] = 0;
+          fetch(32 * d + lane, ents[d], ws[d]);
+        }
         for (int e0 = 0; e0 < n; e0 += 32) {
           const bool have = e0 + lane < n;
-          const uint32_t cent = entA;
-          const uint32_t c0 = wA[0], c1 = wA[1], c2 = wA[2], c3 = wA[3];
-          entA = entB;
+          const uint32_t cent = ents[0];
+          const uint32_t c0 = ws[0][0], c1 = ws[0][1], c2 = ws[0][2], c3 = ws[0][3];
 #pragma unroll
-          for (int i = 0; i < 4; ++i) wA[i] = wB[i];
-          fetch(e0 + 64 + lane, entB, wB);
+          for (int d = 0; d + 1 < kFqDepth; ++d) {
+            ents[d] = ents[d + 1];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) ws[d][i] = ws[d + 1][i];
+          }
+          fetch(e0 + 32 * kFqDepth + lane, ents[kFqDepth - 1], ws[kFqDepth - 1]);
           if (have) {
             const int L = (int)(cent & 31u), blk = (int)(cent >> 5);
             const int nv = tw - 4 * L;                                // valid bytes of that word column
