@@ -203,6 +203,8 @@ def run_ours(args, cfg):
     torch.cuda.synchronize()
 
     names = ["", ""]                                              # kernels the two calls of a step selected
+    # scratch of the FDSC call (its tile dispenser): the caller's, so that the timed calls allocate nothing
+    ws = torch.zeros(max(256, rfim.rfim_workspace_bytes(rfim.OP_FREQ, B, C, S)), dtype=torch.uint8, device=dev)
 
     def step(evs=None):
         if evs:
@@ -211,7 +213,7 @@ def run_ours(args, cfg):
         names[0] = rfim.rfim_last_variant()
         if evs:
             evs[1].record()
-        rfim.rfim_freq_sigma_cut(y, FD_KS, variant=args.fd_variant)
+        rfim.rfim_freq_sigma_cut(y, FD_KS, variant=args.fd_variant, workspace=ws)
         names[1] = rfim.rfim_last_variant()
         if evs:
             evs[2].record()

@@ -31,7 +31,7 @@ constexpr int kFqWarps = 4;
 constexpr int kFqThreads = 32 * kFqWarps;
 constexpr int kFqMaxRing = 4;                        // boxes per warp ring (3 and 5 measured slower)
 constexpr int kFqAhead = 0;                          // L2 prefetch distance in boxes; 0 = off (12 measured: 4.23 vs 3.63 ms)
-constexpr int kFqDepth = 3;                          // repair rounds whose loads are in flight
+constexpr int kFqDepth = 4;                          // repair rounds whose loads are in flight
 constexpr int kFqListCap = 256;                      // candidate blocks per warp and repair chunk
 
 struct __align__(16) FqCtrl {

@@ -32,6 +32,28 @@ bool plan_fd_u8_stream(const Call& c, StreamPlan& pl) {
   return pl.smem <= kMaxSmem;
 }
 
+// The tile dispenser of a launch without caller workspace comes from the device's stream-ordered memory pool.  By
+// default that pool hands all unused memory back to the OS at the next synchronisation, which turns the 256 bytes
+// into an OS round trip per call: keep them (release threshold = maximum), once per device.
+static int ticket_alloc(cudaStream_t stream, unsigned int** out) {
+  static thread_local int prepared_dev = -1;
+  int dev = 0;
+  int st = current_device(dev);
+  if (st != RFIM_OK) return st;
+  if (prepared_dev != dev) {
+    cudaMemPool_t pool;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+      unsigned long long keep = ~0ull;
+      cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
+    }
+    prepared_dev = dev;
+  }
+  void* p = nullptr;
+  CUDA_TRY(cudaMallocAsync(&p, 256, stream));
+  *out = static_cast<unsigned int*>(p);
+  return RFIM_OK;
+}
+
 template <int NCH>
 int launch_fd_stream_n(const Call& c, const StreamPlan& pl, const rfim::FdStreamMaps& maps,
                        const rfim::FdStreamParams& P, int sms) {
@@ -59,9 +81,7 @@ int launch_fd_stream_n(const Call& c, const StreamPlan& pl, const rfim::FdStream
   if (c.workspace) {
     Q.ticket = static_cast<unsigned int*>(c.workspace);
   } else {
-    void* p = nullptr;
-    CUDA_TRY(cudaMallocAsync(&p, 256, c.stream));
-    Q.ticket = static_cast<unsigned int*>(p);
+    if ((st = ticket_alloc(c.stream, &Q.ticket)) != RFIM_OK) return st;
     owned = true;
   }
   cudaError_t e = cudaMemsetAsync(Q.ticket, 0, sizeof(unsigned int), c.stream);
@@ -137,9 +157,7 @@ int launch_fd_quad_n(const Call& c, bool copy, const rfim::FdStreamMaps& maps, c
   if (c.workspace) {
     Q.ticket = static_cast<unsigned int*>(c.workspace);
   } else {
-    void* p = nullptr;
-    CUDA_TRY(cudaMallocAsync(&p, 256, c.stream));
-    Q.ticket = static_cast<unsigned int*>(p);
+    if ((st = ticket_alloc(c.stream, &Q.ticket)) != RFIM_OK) return st;
     owned = true;
   }
   cudaError_t e = cudaMemsetAsync(Q.ticket, 0, sizeof(unsigned int), c.stream);
