@@ -26,7 +26,6 @@
 
 namespace rfim {
 
-constexpr int kFtCols = 32;
 constexpr int kFtWarps = 16;
 constexpr int kFtThreads = 32 * kFtWarps;
 constexpr int kFtCap = 32;
@@ -49,16 +48,22 @@ struct FdF32TileParams {
   int copy;                        // out of place
 };
 
+// COLS = samples per tile: 32 (one CTA per SM) or 16 (tiles of half the size, two CTAs per SM whose loads, sweeps
+// and stores overlap).  A row of the tile is read by COLS lanes: a warp covers 32 / COLS rows at a time and counts as
+// 32 / COLS "virtual warps" of COLS lanes; 512 threads = kFtWarps * 32 / COLS virtual warps.
+template <int COLS>
 struct __align__(16) FtCtrl {
-  double red[kFtWarps][kFtCols][2];
-  uint32_t cred[kFtWarps][kFtCols];
-  uint16_t list[kFtCap][kFtCols];
-  int ln[kFtCols];
-  float med[kFtCols];
+  static constexpr int NVW = kFtWarps * 32 / COLS;
+  double red[NVW][COLS][2];
+  uint32_t cred[NVW][COLS];
+  uint16_t list[kFtCap][COLS];
+  int ln[COLS];
+  float med[COLS];
   uint64_t bar[kFtMaxBoxes];
 };
+template <int COLS>
 __host__ __device__ inline size_t fd_f32_tile_smem_bytes(int C) {
-  return (size_t)C * kFtCols * 4 + sizeof(FtCtrl);
+  return (size_t)C * COLS * 4 + sizeof(FtCtrl<COLS>);
 }
 
 __device__ __forceinline__ void ft_tma_load_2d(void* smem_dst, const CUtensorMap* map, int x, int y, uint64_t* bar) {
@@ -74,12 +79,18 @@ __device__ __forceinline__ void ft_tma_store_2d(const CUtensorMap* map, int x, i
                : "memory");
 }
 
-__global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid_constant__ FdF32TileMaps maps,
-                                                                    const FdF32TileParams P) {
+template <int COLS>
+__global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_kernel(const __grid_constant__ FdF32TileMaps maps,
+                                                                                     const FdF32TileParams P) {
   extern __shared__ __align__(128) uint8_t smem[];
-  float* const tile = reinterpret_cast<float*>(smem);                   // [C][32]
-  FtCtrl* const K = reinterpret_cast<FtCtrl*>(smem + (size_t)P.C * kFtCols * 4);
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  constexpr int kFtCols = COLS;
+  constexpr int NVW = FtCtrl<COLS>::NVW;                                // virtual warps (rows read side by side)
+  float* const tile = reinterpret_cast<float*>(smem);                   // [C][COLS]
+  FtCtrl<COLS>* const K = reinterpret_cast<FtCtrl<COLS>*>(smem + (size_t)P.C * kFtCols * 4);
+  const int tid = threadIdx.x;
+  const int lane = tid & (COLS - 1);                                    // column of the tile
+  const int warp = tid / COLS;                                          // virtual warp: rows warp, warp + NVW, ...
+  const int hwlane = tid & 31;
   const int C = P.C;
   const double rn = 1.0 / (double)C;
   const float inf = __int_as_float(0x7f800000);
@@ -98,7 +109,7 @@ __global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid
     __syncthreads();
     a = 0.0; b = 0.0;
 #pragma unroll
-    for (int w = 0; w < kFtWarps; ++w) { a += K->red[w][lane][0]; b += K->red[w][lane][1]; }
+    for (int w = 0; w < NVW; ++w) { a += K->red[w][lane][0]; b += K->red[w][lane][1]; }
     __syncthreads();
   };
   auto col_sum_u32 = [&](uint32_t v) {
@@ -106,7 +117,7 @@ __global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid
     __syncthreads();
     uint32_t s = 0;
 #pragma unroll
-    for (int w = 0; w < kFtWarps; ++w) s += K->cred[w][lane];
+    for (int w = 0; w < NVW; ++w) s += K->cred[w][lane];
     __syncthreads();
     return s;
   };
@@ -133,13 +144,13 @@ __global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid
       double A0 = 0.0, B0 = 0.0, A1 = 0.0, B1 = 0.0;
       int box = 0;
       int r = warp;
-      for (; r + kFtWarps < C; r += 2 * kFtWarps) {
+      for (; r + NVW < C; r += 2 * NVW) {
         if (first) {
-          const int bx = (r + kFtWarps) / P.box_rows;                    // the later of the two rows
+          const int bx = (r + NVW) / P.box_rows;                    // the later of the two rows
           while (box < bx) { ++box; mbar_wait(&K->bar[box], phase); }
         }
         const double d0 = (double)tile[r * kFtCols + lane] - piv;
-        const double d1 = (double)tile[(r + kFtWarps) * kFtCols + lane] - piv;
+        const double d1 = (double)tile[(r + NVW) * kFtCols + lane] - piv;
         A0 += d0; B0 = fma(d0, d0, B0);
         A1 += d1; B1 = fma(d1, d1, B1);
       }
@@ -187,7 +198,7 @@ __global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid
         if (!(p2 < bb)) p2 = bb;
         if (!(p1 <= p2)) p1 = p2;
         uint32_t c1 = 0, c2 = 0;
-        for (int r = warp; r < C; r += kFtWarps) {
+        for (int r = warp; r < C; r += NVW) {
           const float v = tile[r * kFtCols + lane];
           c1 -= f32f_le_mask(v, p1);
           c2 -= f32f_le_mask(v, p2);
@@ -235,7 +246,7 @@ __global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid
         for (int step = 0; step < 32; ++step) {
           const uint32_t mid = klo + ((khi - klo) >> 1);
           uint32_t cnt = 0;
-          for (int r = warp; r < C; r += kFtWarps) cnt += f32_key(tile[r * kFtCols + lane]) <= mid;
+          for (int r = warp; r < C; r += NVW) cnt += f32_key(tile[r * kFtCols + lane]) <= mid;
           cnt = col_sum_u32(cnt);
           if (cnt > rho) khi = mid; else klo = mid + 1;
         }
@@ -251,14 +262,14 @@ __global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid
       if (warp == 0) K->ln[lane] = 0;
       __syncthreads();
       if (gather) {
-        for (int r = warp; r < C; r += kFtWarps) {
+        for (int r = warp; r < C; r += NVW) {
           const float v = tile[r * kFtCols + lane];
           if (v > a && v <= bb) K->list[atomicAdd(&K->ln[lane], 1)][lane] = (uint16_t)r;
         }
       }
       __syncthreads();
       const uint32_t want = rho - ca;
-      for (uint32_t i = (uint32_t)warp; i < m; i += kFtWarps) {
+      for (uint32_t i = (uint32_t)warp; i < m; i += NVW) {
         const uint32_t ri = K->list[i][lane];
         const float e = tile[ri * kFtCols + lane];
         uint32_t rank = 0;
@@ -289,7 +300,7 @@ __global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid
       double dA = 0.0, dB = 0.0;
       uint32_t cnt = 0;
       if (valid) {
-        for (int r = warp; r < C; r += kFtWarps) {
+        for (int r = warp; r < C; r += NVW) {
           const float v = tile[r * kFtCols + lane];
           if (v > t_hi || v < t_lo) {
             const double d = (double)v - piv;
@@ -304,9 +315,9 @@ __global__ void __launch_bounds__(kFtThreads, 1) fd_f32_tile_kernel(const __grid
       const bool more = it + 1 < P.n_thr;
       if (more || P.counts) {
         const uint32_t total = col_sum_u32(cnt);
-        if (P.counts && warp == 0) {
-          const uint32_t all = __reduce_add_sync(FULL, total);
-          if (lane == 0 && all) atomicAdd(&P.counts[it], (unsigned long long)all);
+        if (P.counts && tid < 32) {                                     // (one copy of every column's total)
+          const uint32_t all = __reduce_add_sync(FULL, hwlane < COLS ? total : 0u);
+          if (hwlane == 0 && all) atomicAdd(&P.counts[it], (unsigned long long)all);
         }
         if (more && __syncthreads_or(total != 0)) {
           col_sum2(dA, dB);

@@ -82,7 +82,11 @@ int try_fd_f32_tile(const Call& c, int sms) {
   const uintptr_t a = reinterpret_cast<uintptr_t>(c.data) | reinterpret_cast<uintptr_t>(c.out);
   if ((a & 15) != 0 || c.stride % 4 != 0) return RFIM_ERR_UNSUPPORTED;          // tensor maps: 16-byte pitch and base
   if (c.channels < 2 || c.channels > 32768) return RFIM_ERR_UNSUPPORTED;
-  const size_t smem = rfim::fd_f32_tile_smem_bytes(c.channels);
+  // tiles of 16 samples when two CTAs then fit an SM (their loads, sweeps and stores overlap), else 32
+  const size_t half = (size_t)(kMaxSmem + 1024) / 2 - 1024;
+  const bool narrow = rfim::fd_f32_tile_smem_bytes<16>(c.channels) <= half;
+  const int cols = narrow ? 16 : 32;
+  const size_t smem = narrow ? rfim::fd_f32_tile_smem_bytes<16>(c.channels) : rfim::fd_f32_tile_smem_bytes<32>(c.channels);
   if (smem > (size_t)kMaxSmem) return RFIM_ERR_UNSUPPORTED;
   if (!tensor_maps_available()) return RFIM_ERR_UNSUPPORTED;
   int box_rows = 0;                                                            // largest divisor of C up to 256
@@ -103,15 +107,15 @@ int try_fd_f32_tile(const Call& c, int sms) {
   P.flags = c.flags;
   P.counts = c.counts;
   P.box_rows = box_rows; P.nboxes = nboxes;
-  P.tiles_per_beam = (c.samples + rfim::kFtCols - 1) / rfim::kFtCols;
+  P.tiles_per_beam = (c.samples + cols - 1) / cols;
   P.total_tiles = (int64_t)P.tiles_per_beam * c.beams;
   P.copy = c.out != c.data ? 1 : 0;
   rfim::FdF32TileMaps maps;
   memset(&maps, 0, sizeof(maps));
   const int64_t rows = (int64_t)c.beams * c.channels;
-  if (!encode_f32_map(P.src, c.stride * 4, c.samples, rows, rfim::kFtCols, box_rows, maps.src)) return RFIM_ERR_UNSUPPORTED;
-  if (!encode_f32_map(P.dst, c.stride * 4, c.samples, rows, rfim::kFtCols, box_rows, maps.dst)) return RFIM_ERR_UNSUPPORTED;
-  auto kernel = rfim::fd_f32_tile_kernel;
+  if (!encode_f32_map(P.src, c.stride * 4, c.samples, rows, cols, box_rows, maps.src)) return RFIM_ERR_UNSUPPORTED;
+  if (!encode_f32_map(P.dst, c.stride * 4, c.samples, rows, cols, box_rows, maps.dst)) return RFIM_ERR_UNSUPPORTED;
+  auto kernel = narrow ? rfim::fd_f32_tile_kernel<16> : rfim::fd_f32_tile_kernel<32>;
   int st = ensure_smem(kernel, smem);
   if (st != RFIM_OK) return st;
   int occ = 0;
