@@ -14,14 +14,15 @@ int launch_fd_u8(const Call& c) {
   if (st != RFIM_OK) return st;
 
   // 0 = auto, 2 = any tuned kernel, 16 = the streaming kernel, 17 = the class-per-warp streaming kernel.
-  // Auto order (measured on B200).  One bin: out of place, or a batch of fewer than about 200 beams,
-  // -> the resident-tile strip kernel first (out of place it writes whole rows from shared memory; on short batches
-  // its tiles need no ticket ramp); large batches in place -> the class-per-warp streaming kernel.  Bins -> the
-  // streaming kernel with per-bin sums.
+  // Auto order (measured on B200 on raw config-3 / config-4 data).  One bin, in place: the resident-
+  // tile strip kernel for short batches (12 beams: 0.153 ms vs 0.170), the class-per-warp streaming kernel from about
+  // 40 beams on (96 beams: 0.93 ms vs 1.07; 240 beams: 2.21 vs 2.61).  Out of place the strip kernel writes whole row
+  // segments from shared memory and stays ahead until about 200 beams (96 beams: 1.76 ms vs 1.89; 240: 4.92 vs
+  // 4.62).  Bins -> the streaming kernel with per-bin sums.
   const bool one_bin = c.bin_size == c.channels;
   const bool tuned = c.variant == 0 || c.variant == 2;
   const int64_t tiles = (int64_t)c.beams * ((c.samples + 127) / 128);
-  if (tuned && one_bin && (c.out != c.data || tiles < 20000)) {
+  if (tuned && one_bin && tiles < (c.out != c.data ? 20000 : 4000)) {
     st = try_fd_u8_strip(c, true, 0, sms);
     if (st != RFIM_ERR_UNSUPPORTED) return st;
   }
