@@ -370,6 +370,8 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
     // Tensor path, full-width tile: the LAST sweep writes the rows it finds clean straight from its registers
     // (F6 fused into F4: no second pass over shared memory for them); repaired rows are written by the repair.
     bool fused_store = false;
+    const bool inplace = P.dst == P.src;
+    uint32_t dirty0 = 0u, dirty1 = 0u;                               // four-row steps some iteration has repaired
     uint8_t* const gds0 = P.dst + ((int64_t)b * C + c0 + row0) * P.stride + s0 + 4 * lane;
     const int64_t rstep = (int64_t)rowmul * P.stride;               // bytes between consecutive rows of this thread
     // ------------------------------------------------------------------ F3..F5: thresholds, on chip
@@ -430,7 +432,8 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
         const bool fuse = kTensor && !need_stats && tw == kStripCols;
         if (fuse) {
           fused_store = true;
-          auto step_store = [&](const uint32_t* c, uint8_t* g) {   // the same test; clean rows go out at once
+          // In place a clean step that no earlier iteration repaired still holds the input: nothing to write.
+          auto step_store = [&](const uint32_t* c, uint8_t* g, bool skip) {   // the same test; clean rows go out at once
             const uint32_t w0 = c[0], w1 = c[RS], w2 = c[2 * RS], w3 = c[3 * RS];
             uint32_t aO = __viaddmax_u16x2(w0, negO, 0u), aE = __viaddmax_u16x2(w0 << 8, negE, 0u);
             uint32_t bO = __viaddmax_u16x2(w1, negO, 0u), bE = __viaddmax_u16x2(w1 << 8, negE, 0u);
@@ -438,7 +441,7 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
             bO = __viaddmax_u16x2(w3, negO, bO); bE = __viaddmax_u16x2(w3 << 8, negE, bE);
             aO = __vimax3_u16x2(aO, bO, thrO); aE = __vimax3_u16x2(aE, bE, thrE);
             const bool h = ((aO ^ thrO) | (aE ^ thrE)) != 0u;
-            if (!h) {
+            if (!h && !skip) {
               *reinterpret_cast<uint32_t*>(g) = w0;
               *reinterpret_cast<uint32_t*>(g + rstep) = w1;
               *reinterpret_cast<uint32_t*>(g + 2 * rstep) = w2;
@@ -449,10 +452,10 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
           uint8_t* g = gds0;
 #pragma unroll 2
           for (; st4 < nA; ++st4, col += 4 * RS, g += 4 * rstep, bit <<= 1)
-            if (step_store(col, g)) hm0 |= bit;
+            if (step_store(col, g, inplace && (dirty0 & bit) == 0u)) hm0 |= bit;
           bit = 1u;
           for (; st4 < n4; ++st4, col += 4 * RS, g += 4 * rstep, bit <<= 1)
-            if (step_store(col, g)) hm1 |= bit;
+            if (step_store(col, g, inplace && (dirty1 & bit) == 0u)) hm1 |= bit;
         } else {
 #pragma unroll 4
           for (; st4 < nA; ++st4, col += 4 * RS, bit <<= 1)
@@ -462,6 +465,8 @@ __global__ void __launch_bounds__(32 * NW, NW == 16 ? 2 : 1) fd_u8_strip_kernel(
             if (step_hits(col)) hm1 |= bit;
         }
         unsigned long long hm = ((unsigned long long)hm1 << 32) | hm0;
+        dirty0 |= slow ? ~0u : hm0;                                   // steps this iteration may modify
+        dirty1 |= slow ? ~0u : hm1;
         int i = 4 * n4;
         for (; i < ni; ++i, col += RS) {
           fix_word(col, col[0], i);
