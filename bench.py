@@ -430,9 +430,11 @@ TABLE_CASES = [
 
 def run_table(quiet: bool = False, only: str = ""):
     """The other BASELINE.json configs (1, 2, 3, 5: the parity-test configurations; the bench line proper is
-    config 4) and the NEXT rows, each timed on its own: 3 warm-ups, 20 timed repetitions on CUDA events, median and
-    best.  Out of place: four rotating buffer pairs, so that no repetition finds its input in L2.  In place: the
-    buffer is restored from a pristine copy and L2 is flushed (a 512 MB write) before every repetition, untimed."""
+    config 4) and the NEXT rows, each timed on its own: 3 warm-ups, 20 timed repetitions, each between its own pair
+    of CUDA events, median and best; the repetitions of a case are enqueued back to back and synchronised once.
+    Out of place: four rotating buffer pairs, so that no repetition finds its input in L2 (a pair comes round again
+    after more than 1 GB of other traffic).  In place: the buffer is restored from a pristine copy and L2 is flushed
+    (a 512 MB write) before every repetition, outside the events."""
     import numpy as np
     import torch
 
@@ -477,13 +479,16 @@ def run_table(quiet: bool = False, only: str = ""):
             if inplace:
                 ys[0].copy_(xs[0])
                 flush.fill_(1)
-        ms = []
+        # all repetitions are enqueued back to back (the device never idles between them, so short kernels are not
+        # timed on a GPU that has just dropped its clocks); every repetition has its own pair of events
+        evs = []
         for i in range(23):
             prepare()
             e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record(); call(i); e1.record(); torch.cuda.synchronize()
-            if i >= 3:
-                ms.append(e0.elapsed_time(e1))
+            e0.record(); call(i); e1.record()
+            evs.append((e0, e1))
+        torch.cuda.synchronize()
+        ms = [a.elapsed_time(b) for (a, b) in evs[3:]]
         med, best = float(np.median(ms)), float(min(ms))
         elems = xs[0].numel()
         es = xs[0].element_size()
