@@ -1,5 +1,7 @@
 // fd_u8_stream.cuh -- frequency-domain sigma cut (FDSC, Fig. 3) for uint8 dynamic spectra:
 // the streaming kernel (8f NEXT-1: the per-bin mean correction of PAPER.md:102,126).
+// Auto mode uses it for requests WITH bins; its one-bin form (kBinned = false, variant 16) has been overtaken by
+// fd_u8_quad.cuh, which keeps this file's geometry, ring and ticket scheme and changes the division of labour.
 //
 // A tile is ALL channels x 128 consecutive samples of one beam.  Unlike a kernel that keeps the tile resident in
 // shared memory, this one streams it ONCE through small per-warp rings and keeps, per thread, only
