@@ -448,6 +448,32 @@ __device__ float f32f_cta_median(int w0, int n, float muf, float sigf, bool need
   return need ? c.req[c.T->rec].result : 0.0f;
 }
 
+// Warp-wide median search for teams narrower than a warp (every lane of the warp calls it): the windows of this
+// warp's teams that need their median are counted by a ballot, the 32 lanes are re-divided evenly among them (32, 16,
+// 8 or 4 lanes per window), each such team runs the search on its window, and the owners pick their result up by a
+// shuffle.  At k = 3 only half of the W = 256 windows need a median: this keeps every lane busy during the search,
+// with no barrier beyond the warp.
+template <int G>
+__device__ float f32f_warp_median(int w0, int n, float muf, float sigf, bool need, F32FastCtx<G>& c) {
+  const int lane = c.lane;
+  const uint32_t lead = __ballot_sync(FULL, need && c.j == 0);     // leaders of the teams that need a median
+  const int K = __popc(lead);                                      // >= 1 (the caller voted)
+  int Gv = 32;
+  while (Gv * K > 32) Gv >>= 1;                                    // K <= 32 / G <= 8, so Gv >= 4
+  const int v = lane / Gv, jv = lane % Gv;
+  const bool act = v < K;
+  const int src = (int)__fns(lead, 0, (act ? v : 0) + 1);          // leader lane of the window this lane works on
+  const int w0v = __shfl_sync(FULL, w0, src), nv = __shfl_sync(FULL, n, src);
+  const float muv = __shfl_sync(FULL, muf, src), sigv = __shfl_sync(FULL, sigf, src);
+  const uint32_t vmask = Gv == 32 ? FULL : (((1u << Gv) - 1u) << (lane & ~(Gv - 1)));
+  F32FastTeam* const Tv = c.T - (lane / G) + (src / G);            // scratch of the team that owns that window
+  const float med = f32f_median_rt(reinterpret_cast<const float4*>(c.slot + w0v), nv, jv, Gv, vmask, Tv, muv, sigv, act);
+  // the window of the team whose leader is lane l was served by virtual team number popc(lead below l)
+  const int mine = __popc(lead & ((1u << (lane & ~(G - 1))) - 1u));
+  const float out = __shfl_sync(FULL, med, mine * Gv);
+  return need ? out : 0.0f;
+}
+
 // One window, all thresholds, by one team.  x4 points at the window in shared memory, n is a multiple of 4; a team
 // without a window (valid = false: more teams than windows in this round) only keeps its warp together.
 // kCta: every team of the CTA is inside this function at the same time (one window per team and row), so the median
@@ -535,7 +561,12 @@ __device__ __forceinline__ void f32f_window(float4* x4, int n, bool valid, const
         if (need_med) { median = med; have_median = true; }
       }
     } else if (f32f_any<G>(need_med)) {
-      const float med = f32f_median<G>(x4, n, Q, (float)mu, (float)sigma, need_med, c);
+      float med;
+      if (G < 32) {
+        med = f32f_warp_median<G>((int)(reinterpret_cast<const float*>(x4) - c.slot), n, (float)mu, (float)sigma, need_med, c);
+      } else {
+        med = f32f_median<G>(x4, n, Q, (float)mu, (float)sigma, need_med, c);
+      }
       if (need_med) { median = med; have_median = true; }
     }
     const float r = P.policy == 0 ? (float)mu : median;
@@ -630,8 +661,10 @@ __global__ void __launch_bounds__(kF32FastThreads, 4) td_f32_fast_kernel(const T
     phase ^= 1;
     // ---------------------------------------------------------------- T2..T5: windows of the row
     uint8_t* fl = P.flags ? P.flags + row * P.S : nullptr;
-    if (G < kF32FastThreads && nwin <= NT && P.policy != 0) {
-      // one window per team: all teams work side by side, the median search is CTA-wide
+    if (G <= 4 && nwin <= NT && P.policy != 0) {
+      // one window per team of 4 lanes (config 5, W = 256: 49 windows on 64 teams): the median search is CTA-wide.
+      // (Teams of 16 lanes re-divide the lanes inside their warp instead -- W = 1024: 0.73 ms against 0.85 ms CTA-wide;
+      // for teams of 4 it is the other way round, 0.87 against 0.83 ms.)
       const int w = c.team;
       const bool valid = w < nwin;
       const int w0 = valid ? w * P.window : 0;
