@@ -376,7 +376,7 @@ __global__ void __launch_bounds__(kFsThreads, 2) fd_u8_stream_kernel(const __gri
           bin += fresh ? 1 : 0;
         }
       }
-      if (2 * NCH < 32) hm &= (1u << (2 * NCH)) - 1u;
+      if (2 * NCH < 32) hm &= (1u << ((2 * NCH) & 31)) - 1u;
 
       // ---- exact repair of the candidate blocks, through global memory (L1 / L2)
       uint32_t cnt4 = 0, sxE = 0, sxO = 0, sq[4] = {0, 0, 0, 0};      // per-column deltas of this thread, packed

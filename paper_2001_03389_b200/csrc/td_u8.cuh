@@ -204,7 +204,6 @@ __global__ void __launch_bounds__(512 * kTeam, 1) td_u8_staged_kernel(const TdU8
   uint32_t phase = 0;
   int xsel = 0;
   const uint4* s4 = reinterpret_cast<const uint4*>(slot);
-  uint32_t* s32 = reinterpret_cast<uint32_t*>(slot);
   const uint4* gmax4 = reinterpret_cast<const uint4*>(gmax);
   const uint4* gmin4 = reinterpret_cast<const uint4*>(gmin);
   const int64_t total_teams = (int64_t)gridDim.x * nteams;
