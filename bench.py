@@ -265,7 +265,7 @@ def run_ours(args, cfg):
     peak, peak_src = hbm_peak()
     td_bytes = 2 * batch_bytes
     fd_bytes = 2 * batch_bytes       # 2 B per uint8 sample, whatever the kernel manages to skip
-    fd_skips_writes = fd_name in ("fd_u8_quad", "fd_u8_stream", "fd_u8_stream_binned")
+    fd_skips_writes = fd_name in ("fd_u8_quad", "fd_u8_stream", "fd_u8_stream_binned", "fd_u8_qbin")
     dom_name, dom_ms, dom_bytes = (td_name, td_ms, td_bytes) if td_ms >= fd_ms else (fd_name, fd_ms, fd_bytes)
     achieved = dom_bytes / (dom_ms * 1e-3) / 1e9
     traffic, traffic_src = ncu_traffic(dom_name, B)

@@ -101,8 +101,9 @@ typedef struct {
                               FDSC only: 13 = strip kernel with per-row bulk copies, 14 = strip kernel in
                               clusters (never the whole tile in one CTA), 15 = strip kernel, 16 = streaming
                               kernel (one bin or bins), 17 = streaming kernel with one warp per alignment
-                              class (one bin).  A variant that cannot run the request, or belongs to the
-                              other operation, returns RFIM_ERR_UNSUPPORTED.                        */
+                              class (one bin), 18 = the same with the per-bin mean correction (bins).
+                              A variant that cannot run the request, or belongs to the other
+                              operation, returns RFIM_ERR_UNSUPPORTED.                              */
   int32_t   reserved;      /* must be 0                                                            */
 } rfim_opts;               /* opts == NULL means all zeros                                          */
 

@@ -20,6 +20,7 @@ VARIANT_AUTO, VARIANT_GENERIC, VARIANT_STAGED = 0, 1, 2
 VARIANT_STAGED_1W, VARIANT_STAGED_2W = 3, 4
 VARIANT_FD_STRIP_BULK, VARIANT_FD_STRIP_CLUSTER, VARIANT_FD_STRIP, VARIANT_FD_STREAM = 13, 14, 15, 16
 VARIANT_FD_QUAD = 17
+VARIANT_FD_QBIN = 18
 OP_TIME, OP_FREQ, OP_TIME_FREQ, OP_HOST = 0, 1, 2, 3
 
 EXPORTS = ("rfim_time_sigma_cut", "rfim_freq_sigma_cut", "rfim_time_freq_sigma_cut", "rfim_sigma_cut_host",

@@ -66,6 +66,7 @@ struct FdStreamParams {
   uint32_t invC;                                   // ceil(2^32 / C)
   int nb, nbins;                                   // binned: channels per bin (multiple of 16), bins
   uint32_t inv_nb, inv_2nb;                        // ceil(2^32 / nb), ceil(2^32 / (2 nb))
+  int off_dst[4];                                  // fd_u8_qbin: the same offsets for the destination's tensor maps
   unsigned int* ticket;                            // tile dispenser of this launch (device, zero before the launch)
 };
 

@@ -134,13 +134,16 @@ bool tensor_maps_available() { return encode_tiled_fn() != nullptr; }
 bool encode_class_maps(const uint8_t* base, int64_t stride, int samples, int64_t rows, int box_w, int box_rows,
                        CUtensorMapL2promotion promo, ClassMaps& out) {
   struct Key { const uint8_t* base; int64_t stride; int samples; int64_t rows; int box_w, box_rows, promo; };
-  thread_local Key last_key = {nullptr, 0, 0, 0, 0, 0, 0};
-  thread_local ClassMaps last_maps;
+  // the two most recent encodings are remembered (a source and a destination buffer per call)
+  thread_local Key last_key[2] = {{nullptr, 0, 0, 0, 0, 0, 0}, {nullptr, 0, 0, 0, 0, 0, 0}};
+  thread_local ClassMaps last_maps[2];
+  thread_local int next_slot = 0;
   Key key;
   memset(&key, 0, sizeof(key));
   key.base = base; key.stride = stride; key.samples = samples; key.rows = rows; key.box_w = box_w;
   key.box_rows = box_rows; key.promo = (int)promo;
-  if (last_key.base != nullptr && memcmp(&last_key, &key, sizeof(Key)) == 0) { out = last_maps; return true; }
+  for (int i = 0; i < 2; ++i)
+    if (last_key[i].base != nullptr && memcmp(&last_key[i], &key, sizeof(Key)) == 0) { out = last_maps[i]; return true; }
   EncodeTiledFn enc = encode_tiled_fn();
   if (!enc) return false;
   for (int k = 0; k < 4; ++k) {
@@ -155,8 +158,9 @@ bool encode_class_maps(const uint8_t* base, int64_t stride, int samples, int64_t
             CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
       return false;
   }
-  last_key = key;
-  last_maps = out;
+  last_key[next_slot] = key;
+  last_maps[next_slot] = out;
+  next_slot ^= 1;
   return true;
 }
 

@@ -103,6 +103,7 @@ int launch_fd_u8(const Call& c);          // launch_fd_misc.cu: variant selectio
 int launch_fd_f32(const Call& c);
 int try_fd_u8_stream(const Call& c, int sms);                              // launch_fd_stream.cu
 int try_fd_u8_quad(const Call& c, int sms);                                // launch_fd_stream.cu
+int try_fd_u8_qbin(const Call& c, int sms);                                // launch_fd_stream.cu
 int try_fd_u8_strip(const Call& c, bool want_tensor, int force_cl, int sms);   // launch_fd_strip.cu
 
 }  // namespace rfim_host

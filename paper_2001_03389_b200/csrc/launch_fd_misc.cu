@@ -13,7 +13,8 @@ int launch_fd_u8(const Call& c) {
   int st = sm_count(sms);
   if (st != RFIM_OK) return st;
 
-  // 0 = auto, 2 = any tuned kernel, 16 = the streaming kernel, 17 = the class-per-warp streaming kernel.
+  // 0 = auto, 2 = any tuned kernel, 16 = the streaming kernel, 17 = the class-per-warp streaming kernel, 18 = its
+  // binned form.
   // Auto order (measured on B200 on raw config-3 / config-4 data).  One bin, in place: the resident-
   // tile strip kernel for short batches (12 beams: 0.153 ms vs 0.170), the class-per-warp streaming kernel from about
   // 40 beams on (96 beams: 0.93 ms vs 1.07; 240 beams: 2.21 vs 2.61).  Out of place the strip kernel writes whole row
@@ -29,6 +30,10 @@ int launch_fd_u8(const Call& c) {
   if (tuned || c.variant == 17) {
     st = try_fd_u8_quad(c, sms);
     if (st != RFIM_ERR_UNSUPPORTED || c.variant == 17) return st;
+  }
+  if (tuned || c.variant == 18) {                     // bins: pooled repair (96 beams, bins of 32: see DESIGN.md 6.2c)
+    st = try_fd_u8_qbin(c, sms);
+    if (st != RFIM_ERR_UNSUPPORTED || c.variant == 18) return st;
   }
   if (tuned || c.variant == 16) {
     st = try_fd_u8_stream(c, sms);

@@ -32,7 +32,7 @@ int validate(int op, void* data, int beams, int channels, int samples, rfim_dtyp
   if (z.reserved != 0) return RFIM_ERR_INVALID;
   if (z.sample_stride != 0 && z.sample_stride < samples) return RFIM_ERR_INVALID;
   if (z.window < 0 || z.bin_size < 0) return RFIM_ERR_INVALID;
-  if (z.variant < 0 || z.variant > 17 || (z.variant >= 5 && z.variant <= 12)) return RFIM_ERR_INVALID;
+  if (z.variant < 0 || z.variant > 18 || (z.variant >= 5 && z.variant <= 12)) return RFIM_ERR_INVALID;
   if (op == 1 && z.bin_size != 0) {
     if (z.bin_size > channels || channels % z.bin_size != 0) return RFIM_ERR_INVALID;
     if (dtype == RFIM_U8 && z.bin_size != channels && z.bin_size > 65536) return RFIM_ERR_INVALID;
@@ -192,7 +192,7 @@ int rfim_time_freq_sigma_cut(void* data, int beams, int channels, int samples, r
   if (st != RFIM_OK) return st;
   st = validate(1, data, beams, channels, samples, dtype, freq_thresholds, n_freq, policy, &o, cf);
   if (st != RFIM_OK) return st;
-  if (variant > 17 || (variant >= 5 && variant <= 12)) return RFIM_ERR_INVALID;
+  if (variant > 18 || (variant >= 5 && variant <= 12)) return RFIM_ERR_INVALID;
   if (variant > 2) return RFIM_ERR_UNSUPPORTED;
   return run_time_freq(ct, cf);
 }

@@ -71,7 +71,7 @@ def test_invalid_arguments_return_minus_one(fn):
     assert call(opts=ctypes.byref(o)) == -1
     o = binding.RfimOpts(); o.reserved = 1
     assert call(opts=ctypes.byref(o)) == -1
-    for v in (18, -1, 7):                                       # 5..12 were the removed cluster variants
+    for v in (19, -1, 7):                                       # 5..12 were the removed cluster variants
         o = binding.RfimOpts(); o.variant = v
         assert call(opts=ctypes.byref(o)) == -1, v
     assert call(data=ctypes.c_void_p(0x1001), dtype=1) == -1   # float32 pointer not 4-byte aligned
@@ -89,7 +89,7 @@ def test_invalid_arguments_return_minus_one(fn):
     # a variant of the other operation is a valid value that this operation cannot run: UNSUPPORTED, decided
     # before anything is enqueued
     if fn == "rfim_time_sigma_cut":
-        for v in (13, 14, 15, 16, 17):
+        for v in (13, 14, 15, 16, 17, 18):
             o = binding.RfimOpts(); o.variant = v
             assert call(opts=ctypes.byref(o)) == -2, v
     elif fn == "rfim_freq_sigma_cut":
@@ -97,7 +97,7 @@ def test_invalid_arguments_return_minus_one(fn):
             o = binding.RfimOpts(); o.variant = v
             assert call(opts=ctypes.byref(o)) == -2, v
     else:
-        for v in (3, 4, 13, 16, 17):
+        for v in (3, 4, 13, 16, 17, 18):
             o = binding.RfimOpts(); o.variant = v
             assert call(opts=ctypes.byref(o)) == -2, v
 

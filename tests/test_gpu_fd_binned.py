@@ -54,7 +54,7 @@ def banded(shape, seed):
 def test_binned_matches_oracle(C, S, nb):
     x = banded((2, C, S), seed=C * 3 + nb)
     name, counts = check(x, [2.75, 2.75], nb)
-    want = ("fd_u8_stream_binned_copy" if (C, nb) == (1536, 32) else "fd_u8_binned_generic" if nb != C
+    want = ("fd_u8_qbin_copy" if (C, nb) == (1536, 32) else "fd_u8_binned_generic" if nb != C
             else "fd_u8_strip1" if S % 4 == 0 else "fd_u8_generic")
     assert name == want
     check(x, [4.0, 3.0, 3.0], nb, inplace=True)
@@ -67,7 +67,7 @@ def test_binned_config3_shape_fig5_parameters():
     cfg = synth.config(3, beams=1, samples=500)
     x = synth.fill_host(cfg)
     name, counts = check(x, [2.75], 32)
-    assert name == "fd_u8_stream_binned_copy" and int(counts[0]) > 0
+    assert name == "fd_u8_qbin_copy" and int(counts[0]) > 0
     check(x, [2.75, 2.75, 2.75], 32, pitch=512)
 
 
