@@ -19,8 +19,9 @@
 //                   threads: lo = ceil((S_b - T) / nb), hi = floor((S_b + T) / nb), r = rounded S_b / nb for every
 //                   (bin, column), four columns per thread;
 //   pass 1 + i      iteration i over the DESTINATION (its own tensor maps): exact per-byte masks against the bounds
-//                   of the block's bin, replaced words stored (nothing else is written), per-bin deltas of S_b and Q
-//                   for the next step.  Branch-free: at 2.75 sigma some lane of a warp has a hit in every block.
+//                   of the block's bin, replaced words stored (nothing else is written), and Q and S_b of the data as
+//                   it now stands for the next step.  Branch-free: at 2.75 sigma some lane of a warp has a hit in
+//                   every block.
 // A CTA is eight warps (alignment class x half of the channels, as many barrier domains as SMs x 3); the rings run
 // across passes and tiles (the first boxes of the next pass are requested while this one ends -- a warp only ever
 // re-reads what it wrote itself, ordered by a proxy fence).  Integer arithmetic is the oracle's
@@ -45,7 +46,7 @@ struct FdQbMaps {
 };
 
 struct __align__(16) QbCtrl {
-  uint32_t acc[kFsCols];                             // Q of 128 columns: totals of pass 0, then deltas
+  uint32_t acc[kFsCols];                             // Q of 128 columns, summed by the pass before a step
   uint32_t T[kFsCols];                               // per-column threshold on |nb x - S_b|
   uint64_t full[kQbWarps][kQbRing];                  // ring mbarriers
   int tk[3][4];                                      // tile tickets handed to this CTA: {tile, beam, tile in beam}
@@ -62,7 +63,7 @@ __device__ __forceinline__ void fence_proxy_async_global() {
 
 // NB = boxes of 8 class rows per warp and tile (C = 64 NB channels); kCopy: out of place
 template <int NB, bool kCopy>
-__global__ void __launch_bounds__(kQbThreads, 2) fd_u8_qbin_kernel(const __grid_constant__ FdQbMaps maps,
+__global__ void __launch_bounds__(kQbThreads, 3) fd_u8_qbin_kernel(const __grid_constant__ FdQbMaps maps,
                                                                   const FdStreamParams P) {
   extern __shared__ __align__(128) uint8_t smem[];
   constexpr int RWC = kFsBoxRows * NB;               // class rows per warp
@@ -124,7 +125,6 @@ __global__ void __launch_bounds__(kQbThreads, 2) fd_u8_qbin_kernel(const __grid_
 
   uint32_t phases = 0;                                // one parity bit per ring slot
   int slot = 0;                                       // ring slot of the next box (boxes follow one another)
-  uint32_t colQ = 0;                                  // thread = column (tid < 128): exact total, kept across iterations
   const int offs = P.off[cls] >> 2, offd = P.off_dst[cls] >> 2;   // word offset of column s0 inside a box row
 
   while (cur_t < P.total_tiles) {
@@ -209,9 +209,8 @@ __global__ void __launch_bounds__(kQbThreads, 2) fd_u8_qbin_kernel(const __grid_
       __syncthreads();                                                // A: Q and bin sums (or their deltas) complete
       if (first && tid == kQbThreads - 1) take_ticket(2);             // the tile after the next one
       if (tid < kFsCols) {
-        const uint32_t q = K->acc[tid];
+        const uint32_t colQ = K->acc[tid];                                           // the pass before this step left the totals
         K->acc[tid] = 0;                                              // read by this thread only
-        if (first) colQ = q; else colQ += q;                          // deltas are modulo 2^32
         uint64_t ss = 0;
         const int sh = (tid & 1) * 16;
         const uint32_t* bp = bS + (tid >> 1);
@@ -241,7 +240,7 @@ __global__ void __launch_bounds__(kQbThreads, 2) fd_u8_qbin_kernel(const __grid_
         for (int bn = warp; bn < nbins; bn += kQbWarps) {
           uint2* const sp2 = reinterpret_cast<uint2*>(bS) + bn * 32 + lane;
           const uint2 sb2 = *sp2;
-          if (!need_stats) *sp2 = make_uint2(0u, 0u);                 // last step: the sums are free for the next tile
+          *sp2 = make_uint2(0u, 0u);                                  // the coming pass (or the next tile) sums afresh
           const uint32_t sbs[4] = {sb2.x & 0xffffu, sb2.x >> 16, sb2.y & 0xffffu, sb2.y >> 16};
           uint32_t lo4 = 0, hi4 = 0, r4 = 0;
 #pragma unroll
@@ -261,14 +260,15 @@ __global__ void __launch_bounds__(kQbThreads, 2) fd_u8_qbin_kernel(const __grid_
       __syncthreads();                                                // B: bounds published
       if (first) { nn_t = K->tk[2][0]; nn_b = K->tk[2][1]; nn_q = K->tk[2][2]; }
 
-      // ---- pass 1 + it over the destination: exact masks, replace, deltas
-      uint32_t cnt_total = 0;
-      uint32_t dQ[4] = {0, 0, 0, 0};                                  // column deltas of Q, all bins
-      uint32_t cnt4 = 0, sx[4] = {0, 0, 0, 0}, sq[4] = {0, 0, 0, 0};  // the bin being streamed: replaced bytes per column
-      uint32_t r4 = 0, chiE = 0, cloE = 0, chiO = 0, cloO = 0;        // its bounds
+      // ---- pass 1 + it over the destination: exact masks, replace, and the sums of the replaced data for the next step
+      uint32_t pc = 0;                                                // 8 x replaced bytes of this lane
+      uint32_t Q4[4] = {0, 0, 0, 0}, B4[4] = {0, 0, 0, 0};
+      uint32_t r4 = 0, chiE = 0, cloE = 0, chiO = 0, cloO = 0;        // bounds of the bin being streamed
       int fbin = bin0, left = bpb;
       bool fresh = true;
-      const uint32_t vm = nvalid >= 4 ? 0xffffffffu : nvalid > 0 ? (1u << (8 * nvalid)) - 1u : 0u;
+      // (bytes beyond the row end are zero-filled and their columns have T = 65535: lo = 0, hi = 255, never cut)
+      const bool want_counts = P.counts != nullptr, want_flags = P.flags != nullptr;
+      uint8_t* gp = dcls;                                             // first row of the coming block
 #pragma unroll 1
       for (int c = 0; c < NB; ++c) {
         mbar_wait(&full[slot], (phases >> slot) & 1u);
@@ -278,7 +278,7 @@ __global__ void __launch_bounds__(kQbThreads, 2) fd_u8_qbin_kernel(const __grid_
 #pragma unroll
         for (int j = 0; j < kFsBoxRows; ++j) w[j] = rowp[j * kFsPitchW];
 #pragma unroll
-        for (int h = 0; h < 2; ++h) {
+        for (int h = 0; h < 2; ++h, gp += 4 * rstep) {
           if (fresh) {                                                // warp-uniform: a new bin starts with this block
             const uint32_t lo4 = lo32[fbin * 32 + lane], hi4 = hi32[fbin * 32 + lane];
             r4 = rr32[fbin * 32 + lane];
@@ -287,68 +287,50 @@ __global__ void __launch_bounds__(kQbThreads, 2) fd_u8_qbin_kernel(const __grid_
             fresh = false;
           }
           const uint32_t c0 = w[4 * h], c1 = w[4 * h + 1], c2 = w[4 * h + 2], c3 = w[4 * h + 3];
-          const uint32_t m0 = bytes_outside_cols(c0, chiE, cloE, chiO, cloO) & vm;
-          const uint32_t m1 = bytes_outside_cols(c1, chiE, cloE, chiO, cloO) & vm;
-          const uint32_t m2 = bytes_outside_cols(c2, chiE, cloE, chiO, cloO) & vm;
-          const uint32_t m3 = bytes_outside_cols(c3, chiE, cloE, chiO, cloO) & vm;
-          if ((m0 | m1 | m2 | m3) != 0u) {
-            uint8_t* const gp = dcls + (int64_t)(kFsBoxRows * c + 4 * h) * rstep;
-            const uint32_t n0 = (c0 & ~m0) | (r4 & m0), n1 = (c1 & ~m1) | (r4 & m1);
-            const uint32_t n2 = (c2 & ~m2) | (r4 & m2), n3 = (c3 & ~m3) | (r4 & m3);
-            if (nvalid >= 4) {
-              if (m0) *reinterpret_cast<uint32_t*>(gp) = n0;
-              if (m1) *reinterpret_cast<uint32_t*>(gp + rstep) = n1;
-              if (m2) *reinterpret_cast<uint32_t*>(gp + 2 * rstep) = n2;
-              if (m3) *reinterpret_cast<uint32_t*>(gp + 3 * rstep) = n3;
-            } else {
-              const uint32_t nn[4] = {n0, n1, n2, n3}, mm[4] = {m0, m1, m2, m3};
-              for (int i = 0; i < 4; ++i)
-                for (int v = 0; v < nvalid; ++v)
-                  if ((mm[i] >> (8 * v)) & 1u) gp[i * rstep + v] = (uint8_t)(nn[i] >> (8 * v));
-            }
-            if (P.flags) {
-              const uint32_t mm[4] = {m0, m1, m2, m3};
-              for (int i = 0; i < 4; ++i) {
-                uint8_t* fl = P.flags + ((int64_t)b * C + 4 * (ywarp + kFsBoxRows * c + 4 * h + i) + cls) * P.S + s0 + 4 * lane;
+          const uint32_t m0 = bytes_outside_cols(c0, chiE, cloE, chiO, cloO);
+          const uint32_t m1 = bytes_outside_cols(c1, chiE, cloE, chiO, cloO);
+          const uint32_t m2 = bytes_outside_cols(c2, chiE, cloE, chiO, cloO);
+          const uint32_t m3 = bytes_outside_cols(c3, chiE, cloE, chiO, cloO);
+          const uint32_t n0 = (c0 & ~m0) | (r4 & m0), n1 = (c1 & ~m1) | (r4 & m1);
+          const uint32_t n2 = (c2 & ~m2) | (r4 & m2), n3 = (c3 & ~m3) | (r4 & m3);
+          if (nvalid >= 4) {
+            if (m0) *reinterpret_cast<uint32_t*>(gp) = n0;
+            if (m1) *reinterpret_cast<uint32_t*>(gp + rstep) = n1;
+            if (m2) *reinterpret_cast<uint32_t*>(gp + 2 * rstep) = n2;
+            if (m3) *reinterpret_cast<uint32_t*>(gp + 3 * rstep) = n3;
+          } else if ((m0 | m1 | m2 | m3) != 0u) {
+            const uint32_t nn[4] = {n0, n1, n2, n3}, mm[4] = {m0, m1, m2, m3};
+            for (int i = 0; i < 4; ++i)
+              for (int v = 0; v < nvalid; ++v)
+                if ((mm[i] >> (8 * v)) & 1u) gp[i * rstep + v] = (uint8_t)(nn[i] >> (8 * v));
+          }
+          if (want_flags && (m0 | m1 | m2 | m3) != 0u) {
+            const uint32_t mm[4] = {m0, m1, m2, m3};
+            for (int i = 0; i < 4; ++i) {
+              uint8_t* fl = P.flags + ((int64_t)b * C + 4 * (ywarp + kFsBoxRows * c + 4 * h + i) + cls) * P.S + s0 + 4 * lane;
 #pragma unroll
-                for (int v = 0; v < 4; ++v)
-                  if ((mm[i] >> (8 * v)) & 1u) fl[v] = 1;
-              }
+              for (int v = 0; v < 4; ++v)
+                if ((mm[i] >> (8 * v)) & 1u) fl[v] = 1;
             }
           }
-          // per column of the bin: how many bytes were replaced, their sum and their sum of squares (branch-free:
-          // at 2.75 sigma some lane has a hit in nearly every block)
-          cnt4 += (m0 & 0x01010101u) + (m1 & 0x01010101u) + (m2 & 0x01010101u) + (m3 & 0x01010101u);   // <= 64 rows per bin
+          if (want_counts) pc += __popc(m0) + __popc(m1) + __popc(m2) + __popc(m3);
           if (need_stats) {
-            const uint32_t f0 = c0 & m0, f1 = c1 & m1, f2 = c2 & m2, f3 = c3 & m3;
-            const uint32_t ab_lo = prmt_b32(f0, f1, 0x5140u), ab_hi = prmt_b32(f0, f1, 0x7362u);
-            const uint32_t cd_lo = prmt_b32(f2, f3, 0x5140u), cd_hi = prmt_b32(f2, f3, 0x7362u);
+            // the next step's statistics are those of the data as it now stands: sum it as pass 0 did (cheaper
+            // than deltas of the replaced bytes, which need their count per column on top)
+            const uint32_t ab_lo = prmt_b32(n0, n1, 0x5140u), ab_hi = prmt_b32(n0, n1, 0x7362u);
+            const uint32_t cd_lo = prmt_b32(n2, n3, 0x5140u), cd_hi = prmt_b32(n2, n3, 0x7362u);
             const uint32_t t0 = prmt_b32(ab_lo, cd_lo, 0x5410u), t1 = prmt_b32(ab_lo, cd_lo, 0x7632u);
             const uint32_t t2 = prmt_b32(ab_hi, cd_hi, 0x5410u), t3 = prmt_b32(ab_hi, cd_hi, 0x7632u);
-            sx[0] = __dp4a(t0, 0x01010101u, sx[0]); sx[1] = __dp4a(t1, 0x01010101u, sx[1]);
-            sx[2] = __dp4a(t2, 0x01010101u, sx[2]); sx[3] = __dp4a(t3, 0x01010101u, sx[3]);
-            sq[0] = __dp4a(t0, t0, sq[0]); sq[1] = __dp4a(t1, t1, sq[1]);
-            sq[2] = __dp4a(t2, t2, sq[2]); sq[3] = __dp4a(t3, t3, sq[3]);
+            B4[0] = __dp4a(t0, 0x01010101u, B4[0]); B4[1] = __dp4a(t1, 0x01010101u, B4[1]);
+            B4[2] = __dp4a(t2, 0x01010101u, B4[2]); B4[3] = __dp4a(t3, 0x01010101u, B4[3]);
+            Q4[0] = __dp4a(t0, t0, Q4[0]); Q4[1] = __dp4a(t1, t1, Q4[1]);
+            Q4[2] = __dp4a(t2, t2, Q4[2]); Q4[3] = __dp4a(t3, t3, Q4[3]);
           }
           if (--left == 0) {                                          // warp-uniform: the bin ends with this block
-            if (cnt4 != 0u) {
-              cnt_total += __dp4a(cnt4, 0x01010101u, 0u);
-              if (need_stats) {
-                uint32_t dS[4];
-#pragma unroll
-                for (int v = 0; v < 4; ++v) {
-                  const uint32_t cn = (cnt4 >> (8 * v)) & 0xffu, r = (r4 >> (8 * v)) & 0xffu;
-                  dS[v] = cn * r - sx[v];                             // modulo 2^32
-                  dQ[v] += cn * r * r - sq[v];
-                  sx[v] = 0; sq[v] = 0;
-                }
-                // two columns per word: plain 32-bit arithmetic is exact because every bin sum is back inside its
-                // 16-bit field once all deltas of the pass are in
-                const uint32_t d01 = dS[0] + (dS[1] << 16), d23 = dS[2] + (dS[3] << 16);
-                if (d01) fs_red_add(&bS[fbin * (kFsCols / 2) + 2 * lane], d01);
-                if (d23) fs_red_add(&bS[fbin * (kFsCols / 2) + 2 * lane + 1], d23);
-              }
-              cnt4 = 0;
+            if (need_stats) {
+              fs_red_add(&bS[fbin * (kFsCols / 2) + 2 * lane], B4[0] | (B4[1] << 16));
+              fs_red_add(&bS[fbin * (kFsCols / 2) + 2 * lane + 1], B4[2] | (B4[3] << 16));
+              B4[0] = 0; B4[1] = 0; B4[2] = 0; B4[3] = 0;
             }
             ++fbin;
             left = bpb;
@@ -364,11 +346,10 @@ __global__ void __launch_bounds__(kQbThreads, 2) fd_u8_qbin_kernel(const __grid_
       }
       if (need_stats) {
 #pragma unroll
-        for (int u = 0; u < 4; ++u)
-          if (dQ[u]) fs_red_add(&K->acc[4 * lane + u], dQ[u]);
+        for (int u = 0; u < 4; ++u) fs_red_add(&K->acc[4 * lane + u], Q4[u]);
       }
       if (P.counts) {
-        cnt_total = __reduce_add_sync(FULL, cnt_total);
+        const uint32_t cnt_total = __reduce_add_sync(FULL, pc >> 3);
         if (lane == 0 && cnt_total) atomicAdd(&P.counts[it], (unsigned long long)cnt_total);
       }
     }

@@ -183,8 +183,17 @@ using QbinKernel = void (*)(const rfim::FdQbMaps, const rfim::FdStreamParams);
 template <int NB>
 int launch_fd_qbin_n(const Call& c, bool copy, const rfim::FdQbMaps& maps, const rfim::FdStreamParams& P, int sms) {
   QbinKernel kernel = copy ? rfim::fd_u8_qbin_kernel<NB, true> : rfim::fd_u8_qbin_kernel<NB, false>;
-  const size_t smem = rfim::fd_qbin_smem_bytes(P.nbins);
+  size_t smem = rfim::fd_qbin_smem_bytes(P.nbins);
   if (smem > (size_t)kMaxSmem) return RFIM_ERR_UNSUPPORTED;
+  // Three CTAs per SM are faster per SM than two (96 beams, bins of 32: 1.70 vs 1.88 ms), but a tile then takes a CTA
+  // a third longer (80 vs 59 us), and a short batch is a handful of tile times: 12 beams are 1176 tiles = 4 full
+  // rounds of 2 x 148 CTAs (0.262 ms) or 2.65 rounds of 3 x 148 (0.290 ms).  Two per SM (asked for through the
+  // shared-memory size) whenever its whole rounds are not more than 4 / 3 of the other's.
+  const size_t two_per_sm = (size_t)(kMaxSmem + 1024) / 3;          // more than a third of an SM's shared memory
+  if (smem < two_per_sm) {
+    const int64_t w2 = (P.total_tiles + 2 * sms - 1) / (2 * sms), w3 = (P.total_tiles + 3 * sms - 1) / (3 * sms);
+    if (3 * w2 <= 4 * w3) smem = two_per_sm;
+  }
   return launch_ticketed(c, copy ? "fd_u8_qbin_copy" : "fd_u8_qbin", kernel, rfim::kQbThreads, smem, maps, P, sms);
 }
 
