@@ -43,14 +43,16 @@
  *
  * Reads around the data: the uint8 FDSC kernels fetch row segments through TMA tensor maps / bulk copies, whose
  * granule is 16 bytes: up to 15 bytes before a row segment and after it (inside the same 16-byte aligned granule,
- * hence inside the same page) are READ and ignored -- also the bytes just before `data` and just behind the last
- * row when those are not 16-byte aligned.  Nothing outside the samples is ever written.
+ * hence inside the same page) are READ and ignored -- also the bytes just before `data` (with bins: and `out`) and
+ * just behind the last row when those are not 16-byte aligned.  Nothing outside the samples is ever written.
  *
  * Performance notes (DESIGN.md section 6 and BASELINE.md section 4 have the numbers).  Tuned kernels exist for:
  *   uint8 TDSC on whole rows of <= 65000 samples, mean or median;
  *   uint8 FDSC, one bin, mean (any channel count that is a multiple of 4) or median (tiles that fit one CTA: up
  *     to about 1570 channels); 512 / 1024 / 1536 / 2048 channels with mean replacement take a streaming kernel on
- *     large in-place batches, and also accept bins whose size is a multiple of 16 and divides channels / 4;
+ *     large in-place batches, and also accept bins whose size is a multiple of 16, at most 256, and divides
+ *     channels / 2 (a kernel that streams the data once per threshold plus once; out of place it reads `out` back
+ *     through tensor maps of its own, with the same 16-byte granule as described above);
  *   float32 TDSC on rows that fit shared memory (<= about 56000 samples) with windows that are multiples of 4
  *     samples (or the whole row), 16-byte aligned rows, mean or median;
  *   float32 FDSC, one bin, mean or median, 16-byte aligned rows, channels x 128 bytes <= about 220 KB.

@@ -1,7 +1,9 @@
 // fd_u8_stream.cuh -- frequency-domain sigma cut (FDSC, Fig. 3) for uint8 dynamic spectra:
 // the streaming kernel (8f NEXT-1: the per-bin mean correction of PAPER.md:102,126).
-// Auto mode uses it for requests WITH bins; its one-bin form (kBinned = false, variant 16) has been overtaken by
-// fd_u8_quad.cuh, which keeps this file's geometry, ring and ticket scheme and changes the division of labour.
+// Reachable as variant 16 only: its one-bin form has been overtaken by fd_u8_quad.cuh, which keeps this file's
+// geometry, ring and ticket scheme and changes the division of labour, its binned form by fd_u8_qbin.cuh, which
+// streams the tile once per threshold step instead of repairing candidate blocks.  Both successors
+// use this file's parameter block, box geometry and helpers.
 //
 // A tile is ALL channels x 128 consecutive samples of one beam.  Unlike a kernel that keeps the tile resident in
 // shared memory, this one streams it ONCE through small per-warp rings and keeps, per thread, only

@@ -17,9 +17,9 @@ int launch_fd_u8(const Call& c) {
   // binned form.
   // Auto order (measured on B200 on raw config-3 / config-4 data).  One bin, in place: the resident-
   // tile strip kernel for short batches (12 beams: 0.153 ms vs 0.170), the class-per-warp streaming kernel from about
-  // 40 beams on (96 beams: 0.93 ms vs 1.07; 240 beams: 2.21 vs 2.61).  Out of place the strip kernel writes whole row
-  // segments from shared memory and stays ahead until about 200 beams (96 beams: 1.76 ms vs 1.89; 240: 4.92 vs
-  // 4.62).  Bins -> the streaming kernel with per-bin sums.
+  // 40 beams on (96 beams: 0.93 ms vs 1.07; 240 beams: 2.21 vs 2.61).  Out of place the strip kernel copies the tile
+  // while its statistics pass reads it and stays ahead until about 200 beams (96 beams: 1.28 ms vs 1.89; 240: 4.48
+  // vs 4.62; 480: 10.2 vs 9.2).  Bins -> one streaming pass per threshold step (fd_u8_qbin.cuh).
   const bool one_bin = c.bin_size == c.channels;
   const bool tuned = c.variant == 0 || c.variant == 2;
   const int64_t tiles = (int64_t)c.beams * ((c.samples + 127) / 128);
