@@ -4,6 +4,7 @@
 #include "fd_u8.cuh"
 #include "fd_f32.cuh"
 #include "fd_f32_tile.cuh"
+#include "fd_f32_bins.cuh"
 #include "fd_u8_binned.cuh"
 
 namespace rfim_host {
@@ -84,7 +85,8 @@ int launch_fd_u8(const Call& c) {
 // ------------------------------------------------------------------------------------------ FD f32
 // the resident-tile kernel (fd_f32_tile.cuh): one bin, all channels x 32 samples per tile in shared memory
 int try_fd_f32_tile(const Call& c, int sms) {
-  if (c.bin_size != c.channels) return RFIM_ERR_UNSUPPORTED;
+  const bool binned = c.bin_size != c.channels;                                 // fd_f32_bins.cuh: a thread owns whole bins
+  if (binned && c.bin_size > 64) return RFIM_ERR_UNSUPPORTED;                   // (one 64-bit flag word per bin)
   const uintptr_t a = reinterpret_cast<uintptr_t>(c.data) | reinterpret_cast<uintptr_t>(c.out);
   if ((a & 15) != 0 || c.stride % 4 != 0) return RFIM_ERR_UNSUPPORTED;          // tensor maps: 16-byte pitch and base
   if (c.channels < 2 || c.channels > 32768) return RFIM_ERR_UNSUPPORTED;
@@ -121,6 +123,19 @@ int try_fd_f32_tile(const Call& c, int sms) {
   const int64_t rows = (int64_t)c.beams * c.channels;
   if (!encode_f32_map(P.src, c.stride * 4, c.samples, rows, cols, box_rows, maps.src)) return RFIM_ERR_UNSUPPORTED;
   if (!encode_f32_map(P.dst, c.stride * 4, c.samples, rows, cols, box_rows, maps.dst)) return RFIM_ERR_UNSUPPORTED;
+  if (binned) {
+    auto bkernel = narrow ? rfim::fd_f32_bins_kernel<16> : rfim::fd_f32_bins_kernel<32>;
+    int st = ensure_smem(bkernel, smem);
+    if (st != RFIM_OK) return st;
+    int occ = 0;
+    if ((st = blocks_per_sm(bkernel, rfim::kFtThreads, smem, occ)) != RFIM_OK) return st;
+    if (occ < 1) return RFIM_ERR_UNSUPPORTED;
+    int64_t grid = P.total_tiles;
+    if (grid > (int64_t)sms * occ) grid = (int64_t)sms * occ;
+    if ((st = clear_outputs(c)) != RFIM_OK) return st;
+    return launch(P.policy ? "fd_f32_bins_median" : "fd_f32_bins", bkernel, dim3((unsigned)grid), dim3(rfim::kFtThreads),
+                  smem, c.stream, 0, maps, P, c.bin_size);
+  }
   auto kernel = narrow ? rfim::fd_f32_tile_kernel<16> : rfim::fd_f32_tile_kernel<32>;
   int st = ensure_smem(kernel, smem);
   if (st != RFIM_OK) return st;

@@ -111,8 +111,8 @@ def test_padded_pitch_and_requests_left_to_the_generic_kernel():
     check(x, [3.0, 3.0], pitch=104, inplace=True, policy="median", want="fd_f32_tile_median")
     check(x, [3.0, 3.0], pitch=101, want="fd_f32_generic")          # rows not 16-byte aligned
     xd = torch.from_numpy(x).to(DEV)
-    rfim.rfim_freq_sigma_cut(xd, [3.0], bin_size=32)                  # bins: the definition kernel
-    assert rfim.rfim_last_variant() == "fd_f32_generic"
+    rfim.rfim_freq_sigma_cut(xd, [3.0], bin_size=32)                  # bins: fd_f32_bins.cuh (its own test module)
+    assert rfim.rfim_last_variant() == "fd_f32_bins"
 
 
 @pytest.mark.parametrize("policy", ["mean", "median"])
