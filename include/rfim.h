@@ -55,11 +55,12 @@
  *     through tensor maps of its own, with the same 16-byte granule as described above);
  *   float32 TDSC on rows that fit shared memory (<= about 56000 samples) with windows that are multiples of 4
  *     samples (or the whole row), 16-byte aligned rows, mean or median;
- *   float32 FDSC, one bin or bins of at most 64 channels, mean or median, 16-byte aligned rows, channels x 64
+ *   float32 FDSC, one bin or bins of at most 64 channels, mean or median, 16-byte aligned rows, channels x 128
  *     bytes <= about 220 KB.
  * Everything else the ABI accepts (uint8 TDSC with windows or rows longer than 65000 samples, uint8 FDSC with median
- * replacement and bins, or odd bin sizes, float32 FDSC with bins of more than 64 channels, unaligned float32 rows) runs in definition
- * kernels (one thread per column / one CTA per row) that go through L2 several times: 10 to 50 times slower.
+ * replacement and bins, or odd bin sizes, float32 FDSC with bins of more than 64 channels, unaligned float32 rows)
+ * runs in definition kernels (one thread per column / one CTA per row) that go through L2 several times: 10 to 50
+ * times slower.
  */
 #ifndef RFIM_H
 #define RFIM_H
