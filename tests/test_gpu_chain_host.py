@@ -67,6 +67,30 @@ def test_chain_other_shapes_policies_and_empty_lists():
     assert e.value.status == -2
 
 
+def test_chain_and_host_path_with_the_papers_parameters():
+    """The pipeline of PAPER.md:126,178 on a config-4 slice: TDSC three times at 3.25 sigma, then FDSC with bins of
+    32 channels twice at 2.75 sigma -- through rfim_time_freq_sigma_cut (the binned streaming kernel behind the
+    composite entry point) and through rfim_sigma_cut_host."""
+    cfg = synth.config(4, beams=3)
+    x = synth.fill_host(cfg, beam0=100, beams=3)
+    tks, fks = [3.25, 3.25, 3.25], [2.75, 2.75]
+    ref, rflags, rcounts = oracle_chain(x, tks, fks, 0, 32)
+    xd = torch.from_numpy(x).to(DEV)
+    out = torch.full_like(xd, 0xAB)
+    flags = torch.full(x.shape, 7, dtype=torch.uint8, device=DEV)
+    counts = torch.full((5,), -1, dtype=torch.int64, device=DEV)
+    rfim.rfim_time_freq_sigma_cut(xd, tks, fks, out=out, bin_size=32, flags=flags, counts=counts)
+    torch.cuda.synchronize()
+    assert rfim.rfim_last_variant() == "fd_u8_qbin"
+    assert np.array_equal(out.cpu().numpy(), ref)
+    assert np.array_equal(flags.cpu().numpy(), rflags)
+    assert counts.cpu().tolist() == rcounts and min(rcounts) > 0
+    h = torch.from_numpy(x.copy()).pin_memory()
+    hout = torch.empty_like(h).pin_memory()
+    rfim.rfim_sigma_cut_host(h, tks, fks, out=hout, bin_size=32)
+    assert np.array_equal(hout.numpy(), ref)
+
+
 def test_chain_float32():
     rng = np.random.default_rng(9)
     x = rng.normal(0, 1, (2, 32, 500)).astype(np.float32)
