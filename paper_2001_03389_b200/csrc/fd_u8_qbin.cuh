@@ -61,8 +61,8 @@ __device__ __forceinline__ void fence_proxy_async_global() {
   asm volatile("fence.proxy.async.global;" ::: "memory");
 }
 
-// NB = boxes of 8 class rows per warp and tile (C = 64 NB channels); kCopy: out of place
-template <int NB, bool kCopy>
+// NB = boxes of 8 class rows per warp and tile (C = 64 NB channels); kCopy: out of place; kOut: flags or counts wanted
+template <int NB, bool kCopy, bool kOut>
 __global__ void __launch_bounds__(kQbThreads, 3) fd_u8_qbin_kernel(const __grid_constant__ FdQbMaps maps,
                                                                   const FdStreamParams P) {
   extern __shared__ __align__(128) uint8_t smem[];
@@ -267,7 +267,7 @@ __global__ void __launch_bounds__(kQbThreads, 3) fd_u8_qbin_kernel(const __grid_
       int fbin = bin0, left = bpb;
       bool fresh = true;
       // (bytes beyond the row end are zero-filled and their columns have T = 65535: lo = 0, hi = 255, never cut)
-      const bool want_counts = P.counts != nullptr, want_flags = P.flags != nullptr;
+      const bool want_counts = kOut && P.counts != nullptr, want_flags = kOut && P.flags != nullptr;
       uint8_t* gp = dcls;                                             // first row of the coming block
 #pragma unroll 1
       for (int c = 0; c < NB; ++c) {
@@ -348,7 +348,7 @@ __global__ void __launch_bounds__(kQbThreads, 3) fd_u8_qbin_kernel(const __grid_
 #pragma unroll
         for (int u = 0; u < 4; ++u) fs_red_add(&K->acc[4 * lane + u], Q4[u]);
       }
-      if (P.counts) {
+      if (want_counts) {
         const uint32_t cnt_total = __reduce_add_sync(FULL, pc >> 3);
         if (lane == 0 && cnt_total) atomicAdd(&P.counts[it], (unsigned long long)cnt_total);
       }

@@ -182,7 +182,9 @@ using QbinKernel = void (*)(const rfim::FdQbMaps, const rfim::FdStreamParams);
 
 template <int NB>
 int launch_fd_qbin_n(const Call& c, bool copy, const rfim::FdQbMaps& maps, const rfim::FdStreamParams& P, int sms) {
-  QbinKernel kernel = copy ? rfim::fd_u8_qbin_kernel<NB, true> : rfim::fd_u8_qbin_kernel<NB, false>;
+  const bool outputs = c.flags != nullptr || c.counts != nullptr;
+  QbinKernel kernel = copy ? (outputs ? rfim::fd_u8_qbin_kernel<NB, true, true> : rfim::fd_u8_qbin_kernel<NB, true, false>)
+                           : (outputs ? rfim::fd_u8_qbin_kernel<NB, false, true> : rfim::fd_u8_qbin_kernel<NB, false, false>);
   size_t smem = rfim::fd_qbin_smem_bytes(P.nbins);
   if (smem > (size_t)kMaxSmem) return RFIM_ERR_UNSUPPORTED;
   // Three CTAs per SM are faster per SM than two (96 beams, bins of 32: 1.70 vs 1.88 ms), but a tile then takes a CTA
