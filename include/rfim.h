@@ -82,7 +82,8 @@ enum {
   RFIM_OK = 0,
   RFIM_ERR_INVALID = -1,     /* bad argument (list below)                                  */
   RFIM_ERR_UNSUPPORTED = -2, /* valid request that no kernel (of the forced variant) runs  */
-  RFIM_ERR_CUDA = -3         /* CUDA runtime error (text: rfim_last_cuda_error)            */
+  RFIM_ERR_CUDA = -3,        /* CUDA runtime error (text: rfim_last_cuda_error)            */
+  RFIM_ERR_TOO_LARGE = -4    /* rfim_freq_sigma_cut_noalloc: beyond RFIM_NOALLOC_MAX_TILES */
 };
 
 /* rfim_workspace_bytes `op` */
@@ -140,6 +141,29 @@ int rfim_time_sigma_cut(void* data, int beams, int channels, int samples, rfim_d
 int rfim_freq_sigma_cut(void* data, int beams, int channels, int samples, rfim_dtype dtype,
                         const double* thresholds, int n_thresholds, rfim_replace policy,
                         const rfim_opts* opts);
+
+/*
+ * FDSC without any device allocation -- the same operation for callers that cannot call
+ * cudaMalloc: code under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  Same
+ * arguments and results as rfim_freq_sigma_cut, restricted to what the streaming kernel covers: RFIM_U8,
+ * RFIM_REPLACE_MEAN, one bin (bin_size 0 or channels), channels in {512, 1024, 1536, 2048}, rows 4-byte aligned
+ * (data, out and the stride multiples of 4) -- anything else is RFIM_ERR_UNSUPPORTED -- and at most
+ * RFIM_NOALLOC_MAX_TILES tiles per call, a tile being 128 samples of one beam:
+ *     beams * ceil(samples / 128) <= RFIM_NOALLOC_MAX_TILES, else RFIM_ERR_TOO_LARGE (nothing is enqueued).
+ * opts->workspace must be NULL and opts->variant 0 (RFIM_ERR_INVALID otherwise): the kernel's scratch, its tile
+ * dispenser, is a static device array of RFIM_NOALLOC_SCRATCH_BYTES bytes inside the library, held by every GPU
+ * that loads the library until the process exits.  The call makes no cudaMalloc / cudaFree / cudaMallocAsync or
+ * other allocating call; it enqueues one 4-byte memset of the dispenser, the clearing of flags / counts if given,
+ * and the kernel on opts->stream.  The first call on a device also looks up the array's device address and the
+ * kernel's launch attributes: make it once outside a stream capture.
+ * All calls on a device share the array: calls that follow one another on a stream are fine, calls that OVERLAP
+ * on the GPU (different streams without a dependency between them) race on the dispenser and give wrong results.
+ */
+#define RFIM_NOALLOC_SCRATCH_BYTES 256
+#define RFIM_NOALLOC_MAX_TILES (1 << 24)
+int rfim_freq_sigma_cut_noalloc(void* data, int beams, int channels, int samples, rfim_dtype dtype,
+                                const double* thresholds, int n_thresholds, rfim_replace policy,
+                                const rfim_opts* opts);
 
 /*
  * TDSC followed by FDSC on its result -- PAPER.md:118,144.  Equivalent to rfim_time_sigma_cut(data -> out)

@@ -15,7 +15,8 @@ from . import build as _build
 
 U8, F32 = 0, 1
 MEAN, MEDIAN = 0, 1
-OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_CUDA = 0, -1, -2, -3
+OK, ERR_INVALID, ERR_UNSUPPORTED, ERR_CUDA, ERR_TOO_LARGE = 0, -1, -2, -3, -4
+NOALLOC_MAX_TILES = 1 << 24                  # include/rfim.h: RFIM_NOALLOC_MAX_TILES
 VARIANT_AUTO, VARIANT_GENERIC, VARIANT_STAGED = 0, 1, 2
 VARIANT_STAGED_1W, VARIANT_STAGED_2W = 3, 4
 VARIANT_FD_STRIP_BULK, VARIANT_FD_STRIP_CLUSTER, VARIANT_FD_STRIP, VARIANT_FD_STREAM = 13, 14, 15, 16
@@ -23,7 +24,8 @@ VARIANT_FD_QUAD = 17
 VARIANT_FD_QBIN = 18
 OP_TIME, OP_FREQ, OP_TIME_FREQ, OP_HOST = 0, 1, 2, 3
 
-EXPORTS = ("rfim_time_sigma_cut", "rfim_freq_sigma_cut", "rfim_time_freq_sigma_cut", "rfim_sigma_cut_host",
+EXPORTS = ("rfim_time_sigma_cut", "rfim_freq_sigma_cut", "rfim_freq_sigma_cut_noalloc", "rfim_time_freq_sigma_cut",
+           "rfim_sigma_cut_host",
            "rfim_workspace_bytes",
            "rfim_launch_count", "rfim_last_variant", "rfim_status_string", "rfim_last_cuda_error",
            "rfim_version")
@@ -68,7 +70,7 @@ def lib() -> ctypes.CDLL:
         dp = ctypes.POINTER(ctypes.c_double)
         sig = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, ctypes.c_int,
                ctypes.c_int, ctypes.POINTER(RfimOpts)]
-        for name in ("rfim_time_sigma_cut", "rfim_freq_sigma_cut"):
+        for name in ("rfim_time_sigma_cut", "rfim_freq_sigma_cut", "rfim_freq_sigma_cut_noalloc"):
             getattr(_lib, name).argtypes = sig
             getattr(_lib, name).restype = ctypes.c_int
         _lib.rfim_time_freq_sigma_cut.argtypes = [ctypes.c_void_p, ctypes.c_int, ctypes.c_int, ctypes.c_int,
@@ -175,6 +177,16 @@ def rfim_freq_sigma_cut(data: torch.Tensor, thresholds: Sequence[float], policy=
     """FDSC.  Asynchronous on `stream`; in place unless `out`."""
     return _call("rfim_freq_sigma_cut", data, thresholds, policy, out, 0, bin_size, flags, counts, stream, variant,
                  workspace)
+
+
+def rfim_freq_sigma_cut_noalloc(data: torch.Tensor, thresholds: Sequence[float], *,
+                                out: Optional[torch.Tensor] = None,
+                                flags: Optional[torch.Tensor] = None, counts: Optional[torch.Tensor] = None,
+                                stream=None) -> torch.Tensor:
+    """FDSC (uint8, one bin, mean) through the entry point that allocates no device memory: its scratch is a static
+    device array inside the library (include/rfim.h).  Calls that overlap on the GPU race on that array."""
+    return _call("rfim_freq_sigma_cut_noalloc", data, thresholds, MEAN, out, 0, 0, flags, counts, stream, VARIANT_AUTO,
+                 None)
 
 
 def rfim_time_freq_sigma_cut(data: torch.Tensor, time_thresholds: Sequence[float], freq_thresholds: Sequence[float],

@@ -306,6 +306,7 @@ const char* rfim_status_string(int status) {
     case RFIM_ERR_INVALID: return "invalid argument";
     case RFIM_ERR_UNSUPPORTED: return "unsupported: no kernel implements this request";
     case RFIM_ERR_CUDA: return "CUDA error (see rfim_last_cuda_error)";
+    case RFIM_ERR_TOO_LARGE: return "too large: more tiles than the fixed scratch of the no-allocation entry point covers (RFIM_NOALLOC_MAX_TILES)";
     default: return "unknown status";
   }
 }
