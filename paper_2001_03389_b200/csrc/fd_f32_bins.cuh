@@ -7,24 +7,25 @@
 // thread reads rows w, w + NVW, ... of its column (coalesced across the lanes of a row, the warps meet in shared
 // memory for every sum); here a thread owns WHOLE BINS of its column -- bins v, v + NVW, ... for virtual warp v -- so
 // that everything the definition asks per bin stays in registers:
-//   step 1  bin mean m_b = (sum of the bin's nb samples) / nb, fp64, in channel order (the oracle's order: the same
-//           bits; odd virtual warps walk their bins backwards so that the two half-warps of a hardware warp never hit
-//           the same banks, which changes the order of THEIR sums and nothing a tolerance of 1e-5 can see);
+//   step 1  bin mean m_b and sum (x - m_b)^2 in ONE fp64 pass around a pivot (the bin's first channel), redone the
+//           long way when the pivot is the outlier; odd virtual warps visit the rows of a bin pairwise swapped so that
+//           the two half-warps of a hardware warp never hit the same banks;
 //   step 2  A = sum (x - m_b), B = sum (x - m_b)^2 over the thread's bins; one shared-memory reduction per column
 //           gives mu' = A / C and sigma'^2 = B / C - mu'^2 (the corrected values are centred: nothing cancels);
-//   step 3  flag <=> |(x - m_b) - mu'| > k sigma' in fp64 as the definition writes it; a flagged sample's ORIGINAL
+//   step 3  flag <=> |x - (m_b + mu')| > k sigma' in fp64, decided by two float bounds per bin that are equivalent to
+//           that test (f32_bounds), so the scan is two float compares per sample; a flagged sample's ORIGINAL
 //           value is replaced by (float) m_b or by the bin's lower median, both taken from the snapshot at the start of
 //           the iteration (the bin is scanned for flags first, replaced afterwards; the median -- rank floor((nb-1)/2)
 //           by counting, O(nb^2) on a bin that has a flagged sample, one bin in six at 2.75 sigma -- before the first
 //           replacement).
-// Every iteration recomputes steps 1-3 from the resident tile (two more passes over shared memory, no deltas).
+// Every iteration recomputes steps 1-3 from the resident tile (two passes over shared memory, no deltas).
 // In place only replaced samples are written; out of place the tile leaves by TMA tensor stores.
 #pragma once
 
 #include <cuda.h>
 
 #include "common.cuh"
-#include "td_f32.cuh"        // f32_key
+#include "td_f32.cuh"        // f32_bounds
 #include "fd_f32_tile.cuh"   // FdF32TileMaps / FdF32TileParams, FtCtrl, ft_tma_* helpers
 
 namespace rfim {
@@ -44,7 +45,11 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_bins_ke
   const int hwlane = tid & 31;
   const int C = P.C, nbins = C / nb;
   const double rn = 1.0 / (double)C, rnb = (double)nb;
-  const bool backwards = (COLS < 32) && (vw & 1);                       // (see the header: bank conflicts)
+  // 16-column tiles: the two half-warps of a hardware warp work on different bins whose rows, nb apart, fall into the
+  // same banks when nb is even; the odd half therefore visits the rows of a bin pairwise swapped (1, 0, 3, 2, ...):
+  // step j is row j ^ 1, reached through two base pointers one row up / down, so that no step costs an instruction
+  const int sw = ((COLS < 32) && (vw & 1) && (nb & 1) == 0) ? 1 : 0;
+  const int skew = sw * COLS;
   if (tid == 0) {
     for (int i = 0; i < P.nboxes; ++i) mbar_init(&K->bar[i], 1);
     fence_mbar_init();
@@ -73,7 +78,7 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_bins_ke
     return s;
   };
   // row of step j (0 .. nb - 1) of a bin that starts at row r0
-  auto row_of = [&](int r0, int j) { return r0 + (backwards ? nb - 1 - j : j); };
+  auto row_of = [&](int r0, int j) { return r0 + (j ^ sw); };
 
   uint32_t phase = 0;
   for (int64_t t = blockIdx.x; t < P.total_tiles; t += gridDim.x) {
@@ -94,25 +99,52 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_bins_ke
     float* const gcol = P.dst + (int64_t)y0 * P.stride + s0 + lane;
     for (int it = 0; it < P.n_thr; ++it) {
       // ---------------------------------------------------------------- steps 1 + 2: bin means, corrected sums
+      // One pass per bin around a pivot (the bin's first channel): Sd = sum (x - x0), Sdd = sum (x - x0)^2 in fp64,
+      // m_b = x0 + Sd / nb, sum (x - m_b)^2 = Sdd - Sd^2 / nb.  Exact enough unless the pivot sits far outside the
+      // bin's spread (it is the outlier): then the bin is summed the long way, mean first.
       double A = 0.0, B = 0.0;
       double mkeep[kFbKeep];                                           // means of the thread's first bins, for step 3
 #pragma unroll
       for (int i = 0; i < kFbKeep; ++i) mkeep[i] = 0.0;
-      if (valid) {
-        int own = 0;
-        for (int bn = vw; bn < nbins; bn += NVW, ++own) {
-          const int r0 = bn * nb;
-          double s = 0.0;
-          for (int j = 0; j < nb; ++j) s += (double)tile[row_of(r0, j) * COLS + lane];
-          const double m = s / rnb;
-#pragma unroll
-          for (int i = 0; i < kFbKeep; ++i)
-            if (own == i) mkeep[i] = m;
-          double a = 0.0, q = 0.0;
+      auto bin_stats = [&](int r0, double& m, double& a, double& q) {
+        const double x0 = (double)tile[r0 * COLS + lane];
+        const float* const pe = tile + r0 * COLS + lane + skew;       // even steps
+        const float* const po = pe - 2 * skew;                        // odd steps
+        double sd = 0.0, sdd = 0.0;
+        int j = 0;
+#pragma unroll 4
+        for (; j + 2 <= nb; j += 2) {
+          const double d0 = (double)pe[j * COLS] - x0, d1 = (double)po[(j + 1) * COLS] - x0;
+          sd += d0; sdd = fma(d0, d0, sdd);
+          sd += d1; sdd = fma(d1, d1, sdd);
+        }
+        if (j < nb) {                                                  // (odd nb: no swap)
+          const double d = (double)pe[j * COLS] - x0;
+          sd += d; sdd = fma(d, d, sdd);
+        }
+        const double md = sd / rnb;
+        m = x0 + md;
+        a = fma(-rnb, md, sd);                                         // sum (x - m_b): rounding residue
+        q = fma(-sd, md, sdd);
+        if (!(q > 1e-6 * sdd)) {                                       // cancellation (or a constant bin): the long way
+          double s1 = 0.0;
+          for (int j = 0; j < nb; ++j) s1 += (double)tile[row_of(r0, j) * COLS + lane];
+          m = s1 / rnb;
+          a = 0.0; q = 0.0;
           for (int j = 0; j < nb; ++j) {
             const double d = (double)tile[row_of(r0, j) * COLS + lane] - m;
             a += d; q = fma(d, d, q);
           }
+        }
+      };
+      if (valid) {
+        int own = 0;
+        for (int bn = vw; bn < nbins; bn += NVW, ++own) {
+          double m, a, q;
+          bin_stats(bn * nb, m, a, q);
+#pragma unroll
+          for (int i = 0; i < kFbKeep; ++i)
+            if (own == i) mkeep[i] = m;
           A += a; B += q;
         }
       }
@@ -122,6 +154,8 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_bins_ke
       if (!(var > 0.0)) var = 0.0;
       const double cut = P.k[it] * sqrt(var);
       // ---------------------------------------------------------------- step 3: flag, replace (own bins only)
+      // flag <=> |x - (m_b + mu')| > k sigma' in fp64, taken as two float bounds per bin that decide exactly that
+      // (f32_bounds): the scan of a bin is two float compares per sample
       uint32_t cnt = 0;
       if (valid) {
         int own = 0;
@@ -132,18 +166,30 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_bins_ke
 #pragma unroll
             for (int i = 0; i < kFbKeep; ++i)
               if (own == i) m = mkeep[i];
-          } else {                                                     // (many small bins: summed again, same order)
-            double s = 0.0;
-            for (int j = 0; j < nb; ++j) s += (double)tile[row_of(r0, j) * COLS + lane];
-            m = s / rnb;
+          } else {                                                     // (many small bins: summed again)
+            double a, q;
+            bin_stats(r0, m, a, q);
           }
+          float t_lo, t_hi;
+          f32_bounds(m + mu, cut, t_lo, t_hi);
           // scan the snapshot first: bit j <=> the sample of step j is flagged (nb <= 64: host-checked)
           {
-            unsigned long long fm = 0ull;
-            for (int j = 0; j < nb; ++j) {
-              const double d = ((double)tile[row_of(r0, j) * COLS + lane] - m) - mu;
-              if (fabs(d) > cut) fm |= 1ull << j;
+            const float* const pe = tile + r0 * COLS + lane + skew;
+            const float* const po = pe - 2 * skew;
+            uint32_t f0 = 0u, f1 = 0u;                                  // steps 0..31 and 32..63
+            int j = 0;
+#pragma unroll 4
+            for (; j + 2 <= nb; j += 2) {
+              const float v0 = pe[j * COLS], v1 = po[(j + 1) * COLS];
+              const uint32_t h = ((v0 > t_hi || v0 < t_lo) ? 1u : 0u) | ((v1 > t_hi || v1 < t_lo) ? 2u : 0u);
+              if (j < 32) f0 |= h << (j & 31); else f1 |= h << (j & 31);
             }
+            if (j < nb) {
+              const float v = pe[j * COLS];
+              const uint32_t h = (v > t_hi || v < t_lo) ? 1u : 0u;
+              if (j < 32) f0 |= h << (j & 31); else f1 |= h << (j & 31);
+            }
+            unsigned long long fm = ((unsigned long long)f1 << 32) | f0;
             if (fm == 0ull) continue;
             float rv = (float)m;
             if (P.policy != 0) {
