@@ -47,6 +47,7 @@ struct __align__(8) F32FastSel { int w0, n; float mu, sig, result; int pad; };
 struct __align__(16) F32FastXchg {
   double red[2][8][2];
   uint32_t redu[2][8];
+  uint16_t biglist[64];             // gather list of a wide team (f32f_cap<G>() = 64 for G >= 64)
 };
 __host__ __device__ constexpr int f32_fast_teams(int G) { return kF32FastThreads / G; }
 __host__ __device__ inline size_t f32_fast_smem_bytes(int S, int G) {
@@ -142,7 +143,7 @@ __device__ __forceinline__ void f32f_each_quad(const F32Quads& q, int j, F&& bod
 }
 // elements a team gathers and ranks at the end of the median search: the ranking costs m^2 / G compares per lane
 template <int G>
-__host__ __device__ constexpr int f32f_cap() { return G <= 4 ? 12 : (G <= 16 ? 16 : 32); }
+__host__ __device__ constexpr int f32f_cap() { return G <= 4 ? 12 : (G <= 16 ? 16 : (G <= 32 ? 32 : 64)); }
 
 // Teams narrower than a warp run side by side in one warp.  Their heavy loops must stay CONVERGED (a warp that
 // splits into its teams executes every loop once per team), so the control flow around them is warp-uniform: every
@@ -159,6 +160,9 @@ template <int G>
 __device__ float f32f_median(const float4* x4, int n, const F32Quads& Q, float muf, float sigf, bool need,
                              F32FastCtx<G>& c) {
   constexpr uint32_t CAP = (uint32_t)f32f_cap<G>();
+  // Wide teams gather up to 64 candidates: with n = 12500 the second counting pass leaves 36 +- 6 of them, and a cap
+  // of 32 meant a third pass over the row nearly every time.
+  uint16_t* const list = G > 32 ? c.X->biglist : c.T->list;
   const float* x = reinterpret_cast<const float*>(x4);
   const uint32_t rho = need ? (uint32_t)(n - 1) >> 1 : 0u;
   const float inf = __int_as_float(0x7f800000);
@@ -264,21 +268,21 @@ __device__ float f32f_median(const float4* x4, int n, const F32Quads& Q, float m
       const float4 v = x4[qi];
       const bool in0 = v.x > a && v.x <= b, in1 = v.y > a && v.y <= b, in2 = v.z > a && v.z <= b, in3 = v.w > a && v.w <= b;
       if (in0 | in1 | in2 | in3) {
-        if (in0) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi);
-        if (in1) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 1);
-        if (in2) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 2);
-        if (in3) c.T->list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 3);
+        if (in0) list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi);
+        if (in1) list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 1);
+        if (in2) list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 2);
+        if (in3) list[atomicAdd(&c.T->ln, 1)] = (uint16_t)(4 * qi + 3);
       }
     });
   }
   f32f_sync<G>(c);
   const uint32_t want = rho - ca;
   for (uint32_t i = (uint32_t)c.j; i < m; i += G) {
-    const uint32_t ii = c.T->list[i];
+    const uint32_t ii = list[i];
     const float e = x[ii];
     uint32_t rank = 0;
     for (uint32_t k = 0; k < m; ++k) {
-      const uint32_t kk = c.T->list[k];
+      const uint32_t kk = list[k];
       const float o = x[kk];
       rank += (o < e) || (o == e && kk < ii);
     }
@@ -295,7 +299,10 @@ __device__ float f32f_median(const float4* x4, int n, const F32Quads& Q, float m
 __device__ inline float f32f_median_rt(const float4* x4, int n, int jv, int Gv, uint32_t vmask, F32FastTeam* T, float muf,
                                 float sigf, bool act) {
   const float* x = reinterpret_cast<const float*>(x4);
-  const uint32_t CAP = Gv <= 4 ? 12u : (Gv <= 16 ? 16u : 32u);
+  // Gathering m candidates and ranking them costs about 5 m^2 / Gv instructions per lane, one more counting pass about
+  // 3.5 n / Gv: the cap follows the window length (after the second pass m is 15 +- 4 for n = 256, 20 +- 4.5 for 1024;
+  // measured: W = 1024 0.734 -> 0.727 ms with 26 instead of 16, W = 256 best with 12 / 16)
+  const uint32_t CAP = n <= 256 ? (Gv <= 4 ? 12u : 16u) : (n <= 1024 ? 26u : 32u);
   const int nq = act ? n >> 2 : 0;
   const uint32_t rho = act ? (uint32_t)(n - 1) >> 1 : 0u;
   const float inf = __int_as_float(0x7f800000);
