@@ -59,21 +59,34 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_bins_ke
   __syncthreads();
 
   // sum of two doubles per column over the virtual warps (result in every thread of the column)
+  // (16 columns: the two virtual warps of a hardware warp hold the same columns and meet by a shuffle first)
+  constexpr int NRED = COLS == 16 ? NVW / 2 : NVW;
   auto col_sum2 = [&](double& a, double& b) {
-    K->red[vw][lane][0] = a;
-    K->red[vw][lane][1] = b;
+    if (COLS == 16) {
+      a += __shfl_xor_sync(FULL, a, 16);
+      b += __shfl_xor_sync(FULL, b, 16);
+      if ((vw & 1) == 0) { K->red[vw >> 1][lane][0] = a; K->red[vw >> 1][lane][1] = b; }
+    } else {
+      K->red[vw][lane][0] = a;
+      K->red[vw][lane][1] = b;
+    }
     __syncthreads();
     a = 0.0; b = 0.0;
 #pragma unroll
-    for (int w = 0; w < NVW; ++w) { a += K->red[w][lane][0]; b += K->red[w][lane][1]; }
+    for (int w = 0; w < NRED; ++w) { a += K->red[w][lane][0]; b += K->red[w][lane][1]; }
     __syncthreads();
   };
   auto col_sum_u32 = [&](uint32_t v) {
-    K->cred[vw][lane] = v;
+    if (COLS == 16) {
+      v += __shfl_xor_sync(FULL, v, 16);
+      if ((vw & 1) == 0) K->cred[vw >> 1][lane] = v;
+    } else {
+      K->cred[vw][lane] = v;
+    }
     __syncthreads();
     uint32_t s = 0;
 #pragma unroll
-    for (int w = 0; w < NVW; ++w) s += K->cred[w][lane];
+    for (int w = 0; w < NRED; ++w) s += K->cred[w][lane];
     __syncthreads();
     return s;
   };

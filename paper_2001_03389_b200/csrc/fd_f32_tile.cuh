@@ -103,21 +103,35 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_ke
   __syncthreads();
 
   // sum of two doubles per column over the 16 warps (result in every thread of the column)
+  // (16 columns: the two virtual warps of a hardware warp hold the same columns and meet by a shuffle first, which
+  // halves the partial sums every thread has to add up)
+  constexpr int NRED = COLS == 16 ? NVW / 2 : NVW;
   auto col_sum2 = [&](double& a, double& b) {
-    K->red[warp][lane][0] = a;
-    K->red[warp][lane][1] = b;
+    if (COLS == 16) {
+      a += __shfl_xor_sync(FULL, a, 16);
+      b += __shfl_xor_sync(FULL, b, 16);
+      if ((warp & 1) == 0) { K->red[warp >> 1][lane][0] = a; K->red[warp >> 1][lane][1] = b; }
+    } else {
+      K->red[warp][lane][0] = a;
+      K->red[warp][lane][1] = b;
+    }
     __syncthreads();
     a = 0.0; b = 0.0;
 #pragma unroll
-    for (int w = 0; w < NVW; ++w) { a += K->red[w][lane][0]; b += K->red[w][lane][1]; }
+    for (int w = 0; w < NRED; ++w) { a += K->red[w][lane][0]; b += K->red[w][lane][1]; }
     __syncthreads();
   };
   auto col_sum_u32 = [&](uint32_t v) {
-    K->cred[warp][lane] = v;
+    if (COLS == 16) {
+      v += __shfl_xor_sync(FULL, v, 16);
+      if ((warp & 1) == 0) K->cred[warp >> 1][lane] = v;
+    } else {
+      K->cred[warp][lane] = v;
+    }
     __syncthreads();
     uint32_t s = 0;
 #pragma unroll
-    for (int w = 0; w < NVW; ++w) s += K->cred[w][lane];
+    for (int w = 0; w < NRED; ++w) s += K->cred[w][lane];
     __syncthreads();
     return s;
   };
@@ -142,12 +156,11 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_ke
     double A = 0.0, B = 0.0;
     auto sums = [&](bool first) {
       double A0 = 0.0, B0 = 0.0, A1 = 0.0, B1 = 0.0;
-      int box = 0;
+      int box = 0, box_end = P.box_rows;                              // rows below box_end have landed
       int r = warp;
       for (; r + NVW < C; r += 2 * NVW) {
         if (first) {
-          const int bx = (r + NVW) / P.box_rows;                    // the later of the two rows
-          while (box < bx) { ++box; mbar_wait(&K->bar[box], phase); }
+          while (r + NVW >= box_end) { ++box; box_end += P.box_rows; mbar_wait(&K->bar[box], phase); }   // the later row
         }
         const double d0 = (double)tile[r * kFtCols + lane] - piv;
         const double d1 = (double)tile[(r + NVW) * kFtCols + lane] - piv;
@@ -156,8 +169,7 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_ke
       }
       if (r < C) {
         if (first) {
-          const int bx = r / P.box_rows;
-          while (box < bx) { ++box; mbar_wait(&K->bar[box], phase); }
+          while (r >= box_end) { ++box; box_end += P.box_rows; mbar_wait(&K->bar[box], phase); }
         }
         const double d0 = (double)tile[r * kFtCols + lane] - piv;
         A0 += d0; B0 = fma(d0, d0, B0);
