@@ -154,28 +154,33 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_ke
     mbar_wait(&K->bar[0], phase);
     double piv = (double)tile[lane];                                     // row 0 of the column
     double A = 0.0, B = 0.0;
+    // rows warp, warp + NVW, ... of the column, eight per trip at compile-time offsets; the first pass follows the
+    // tensor boxes as they land (one wait per box instead of a check per row)
+    constexpr int RSTEP = NVW * kFtCols;                               // floats between consecutive rows of a thread
+    const float* const pcol = tile + warp * kFtCols + lane;
+    const int nrows = C > warp ? (C - warp + NVW - 1) / NVW : 0;       // rows of this thread
     auto sums = [&](bool first) {
       double A0 = 0.0, B0 = 0.0, A1 = 0.0, B1 = 0.0;
-      int box = 0, box_end = P.box_rows;                              // rows below box_end have landed
-      int r = warp;
-      for (; r + NVW < C; r += 2 * NVW) {
-        if (first) {
-          while (r + NVW >= box_end) { ++box; box_end += P.box_rows; mbar_wait(&K->bar[box], phase); }   // the later row
+      int i = 0;
+      for (int box = 0; box < P.nboxes; ++box) {
+        if (first && box > 0) mbar_wait(&K->bar[box], phase);
+        // rows of this thread below the end of the box: warp + NVW i < (box + 1) box_rows
+        const int lim = box + 1 == P.nboxes ? nrows : min(nrows, max(0, ((box + 1) * P.box_rows - warp + NVW - 1) / NVW));
+        const float* q = pcol + (size_t)i * RSTEP;
+#pragma unroll 1
+        for (; i + 8 <= lim; i += 8, q += 8 * RSTEP) {
+#pragma unroll
+          for (int u = 0; u < 8; u += 2) {
+            const double d0 = (double)q[u * RSTEP] - piv, d1 = (double)q[(u + 1) * RSTEP] - piv;
+            A0 += d0; B0 = fma(d0, d0, B0);
+            A1 += d1; B1 = fma(d1, d1, B1);
+          }
         }
-        const double d0 = (double)tile[r * kFtCols + lane] - piv;
-        const double d1 = (double)tile[(r + NVW) * kFtCols + lane] - piv;
-        A0 += d0; B0 = fma(d0, d0, B0);
-        A1 += d1; B1 = fma(d1, d1, B1);
-      }
-      if (r < C) {
-        if (first) {
-          while (r >= box_end) { ++box; box_end += P.box_rows; mbar_wait(&K->bar[box], phase); }
+        for (; i < lim; ++i, q += RSTEP) {
+          const double d0 = (double)q[0] - piv;
+          A0 += d0; B0 = fma(d0, d0, B0);
         }
-        const double d0 = (double)tile[r * kFtCols + lane] - piv;
-        A0 += d0; B0 = fma(d0, d0, B0);
       }
-      if (first)
-        while (box + 1 < P.nboxes) { ++box; mbar_wait(&K->bar[box], phase); }   // every box has landed for this thread
       A = A0 + A1; B = B0 + B1;
       col_sum2(A, B);
     };
@@ -210,10 +215,23 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_ke
         if (!(p2 < bb)) p2 = bb;
         if (!(p1 <= p2)) p1 = p2;
         uint32_t c1 = 0, c2 = 0;
-        for (int r = warp; r < C; r += NVW) {
-          const float v = tile[r * kFtCols + lane];
-          c1 -= f32f_le_mask(v, p1);
-          c2 -= f32f_le_mask(v, p2);
+        {
+          const float* q = pcol;
+          int i = 0;
+#pragma unroll 1
+          for (; i + 8 <= nrows; i += 8, q += 8 * RSTEP) {
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              const float v = q[u * RSTEP];
+              c1 -= f32f_le_mask(v, p1);
+              c2 -= f32f_le_mask(v, p2);
+            }
+          }
+          for (; i < nrows; ++i, q += RSTEP) {
+            const float v = q[0];
+            c1 -= f32f_le_mask(v, p1);
+            c2 -= f32f_le_mask(v, p2);
+          }
         }
         const uint32_t packed = col_sum_u32(c1 | (c2 << 16));            // C <= 2^15 (host-checked)
         if (searching) {
@@ -274,9 +292,30 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_ke
       if (warp == 0) K->ln[lane] = 0;
       __syncthreads();
       if (gather) {
-        for (int r = warp; r < C; r += NVW) {
-          const float v = tile[r * kFtCols + lane];
-          if (v > a && v <= bb) K->list[atomicAdd(&K->ln[lane], 1)][lane] = (uint16_t)r;
+        for (int i0 = 0; i0 < nrows; i0 += 32) {                          // scan into a mask, then append the few hits
+          const float* q = pcol + (size_t)i0 * RSTEP;
+          const int n32 = min(32, nrows - i0);
+          uint32_t fm = 0u;
+          int i = 0;
+#pragma unroll 1
+          for (; i + 8 <= n32; i += 8, q += 8 * RSTEP) {
+            uint32_t h = 0u;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              const float v = q[u * RSTEP];
+              h |= (v > a && v <= bb) ? (1u << u) : 0u;
+            }
+            fm |= h << i;
+          }
+          for (; i < n32; ++i, q += RSTEP) {
+            const float v = q[0];
+            if (v > a && v <= bb) fm |= 1u << i;
+          }
+          while (fm) {
+            const int j = __ffs((int)fm) - 1;
+            fm &= fm - 1u;
+            K->list[atomicAdd(&K->ln[lane], 1)][lane] = (uint16_t)(warp + NVW * (i0 + j));
+          }
         }
       }
       __syncthreads();
@@ -312,10 +351,31 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_ke
       double dA = 0.0, dB = 0.0;
       uint32_t cnt = 0;
       if (valid) {
-        for (int r = warp; r < C; r += NVW) {
-          const float v = tile[r * kFtCols + lane];
-          if (v > t_hi || v < t_lo) {
-            const double d = (double)v - piv;
+        // scan 32 rows at a time into a bit mask (unrolled, compile-time offsets), then visit the few flagged rows
+        for (int i0 = 0; i0 < nrows; i0 += 32) {
+          const float* q = pcol + (size_t)i0 * RSTEP;
+          const int n32 = min(32, nrows - i0);
+          uint32_t fm = 0u;
+          int i = 0;
+#pragma unroll 1
+          for (; i + 8 <= n32; i += 8, q += 8 * RSTEP) {
+            uint32_t h = 0u;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+              const float v = q[u * RSTEP];
+              h |= (v > t_hi || v < t_lo) ? (1u << u) : 0u;
+            }
+            fm |= h << i;
+          }
+          for (; i < n32; ++i, q += RSTEP) {
+            const float v = q[0];
+            if (v > t_hi || v < t_lo) fm |= 1u << i;
+          }
+          while (fm) {
+            const int j = __ffs((int)fm) - 1;
+            fm &= fm - 1u;
+            const int r = warp + NVW * (i0 + j);
+            const double d = (double)tile[r * kFtCols + lane] - piv;
             dA += dr - d; dB += dr * dr - d * d;
             tile[r * kFtCols + lane] = rv;
             if (!P.copy) gcol[(int64_t)r * P.stride] = rv;
