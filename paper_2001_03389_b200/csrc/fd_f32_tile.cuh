@@ -359,13 +359,18 @@ __global__ void __launch_bounds__(kFtThreads, COLS == 32 ? 1 : 2) fd_f32_tile_ke
           int i = 0;
 #pragma unroll 1
           for (; i + 8 <= n32; i += 8, q += 8 * RSTEP) {
-            uint32_t h = 0u;
+            // eight rows at once through their largest and smallest value (FMNMX3): 2 % of the groups hold a hit at 3 sigma
+            float v[8];
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-              const float v = q[u * RSTEP];
-              h |= (v > t_hi || v < t_lo) ? (1u << u) : 0u;
+            for (int u = 0; u < 8; ++u) v[u] = q[u * RSTEP];
+            const float mx = fmaxf(fmaxf(fmaxf(v[0], v[1]), fmaxf(v[2], v[3])), fmaxf(fmaxf(v[4], v[5]), fmaxf(v[6], v[7])));
+            const float mn = fminf(fminf(fminf(v[0], v[1]), fminf(v[2], v[3])), fminf(fminf(v[4], v[5]), fminf(v[6], v[7])));
+            if (mx > t_hi || mn < t_lo) {
+              uint32_t h = 0u;
+#pragma unroll
+              for (int u = 0; u < 8; ++u) h |= (v[u] > t_hi || v[u] < t_lo) ? (1u << u) : 0u;
+              fm |= h << i;
             }
-            fm |= h << i;
           }
           for (; i < n32; ++i, q += RSTEP) {
             const float v = q[0];
